@@ -1,0 +1,26 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on the B200 box)")
+
+
+@pytest.fixture(scope="session")
+def problems():
+    """Cache of generated configs shared by the whole session."""
+    import cg_inputs
+    cache = {}
+
+    def get(cfg, grid=None):
+        key = (cfg, grid)
+        if key not in cache:
+            cache[key] = cg_inputs.make_config(cfg, grid)
+        return cache[key]
+    return get

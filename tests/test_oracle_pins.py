@@ -1,0 +1,325 @@
+"""Pins of the CPU oracle against things other than itself (SURVEY.md 8(c) pin table).
+
+Each test names the mistake it would catch.  No value here comes from the CUDA path.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import cg_inputs as gi
+from oracle import cg_oracle as orc
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _dense(rp, ci, va):
+    n = len(rp) - 1
+    A = np.zeros((n, n))
+    for i in range(n):
+        for k in range(rp[i], rp[i + 1]):
+            A[i, ci[k]] += va[k]
+    return A
+
+
+def _golden(name):
+    out = {}
+    with open(os.path.join(GOLDEN, name)) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, *v = line.split()
+            out[k] = np.array([float(t) for t in v])
+    return out
+
+
+# ---------------------------------------------------------------- SpMV / dot
+
+@pytest.mark.parametrize("n", [3, 5, 8])
+def test_spmv_vs_bruteforce_dense(n):
+    """Brute-force dense mat-vec with long-double accumulation: catches a wrong index,
+    a transposed operand (A is made non-symmetric here), a dropped last entry."""
+    rp, ci, va = gi.stencil27(n)
+    va = va * (1.0 + 0.25 * gi.hash_uniform(9, 2, np.arange(len(va), dtype=np.uint64)))  # break symmetry
+    A = _dense(rp, ci, va).astype(np.longdouble)
+    x = gi.seeded_vector(7, n ** 3)
+    want = np.array([np.sum(A[i] * x.astype(np.longdouble)) for i in range(n ** 3)], dtype=np.longdouble)
+    denom = orc.absrow(rp, ci, va, x)
+    for got in (orc.spmv(rp, ci, va, x), orc.spmv_ld(rp, ci, va, x)):
+        assert np.all(np.abs(got - want.astype(np.float64)) <= 3e-15 * denom)
+    # absrow against its definition
+    np.testing.assert_allclose(denom, np.abs(_dense(rp, ci, va)) @ np.abs(x), rtol=1e-14)
+
+
+def test_spmv_unsorted_and_duplicate_columns():
+    """CSR contract (include/cg.h): columns need not be sorted or unique; duplicates add."""
+    rp = np.array([0, 3, 5], dtype=np.int32)
+    ci = np.array([1, 0, 1, 1, 0], dtype=np.int32)
+    va = np.array([2.0, 3.0, 4.0, 5.0, 7.0])
+    y = orc.spmv(rp, ci, va, np.array([10.0, 100.0]))
+    assert y.tolist() == [2 * 100 + 3 * 10 + 4 * 100, 5 * 100 + 7 * 10]
+
+
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_row_sums_are_one_hundredth(problems, cfg):
+    """A*1 = 0.01*1: the matrix is a weighted graph Laplacian + 0.01 I (generator + SpMV)."""
+    p = problems(cfg)
+    ones = np.ones(p.n)
+    y = orc.spmv(p.rowptr, p.colind, p.vals, ones)
+    tol = 1e-13 * orc.absrow(p.rowptr, p.colind, p.vals, ones)
+    assert np.all(np.abs(y - 0.01) <= tol)
+
+
+def test_row_sums_contrast_scaled_down():
+    p = gi.make_config(4, grid=24)
+    ones = np.ones(p.n)
+    y = orc.spmv(p.rowptr, p.colind, p.vals, ones)
+    assert np.all(np.abs(y - 0.01) <= 1e-13 * orc.absrow(p.rowptr, p.colind, p.vals, ones))
+    assert p.vals.max() > 1000.0            # the cylinder is really there
+
+
+def test_oracle_spmv_matches_generator_rhs(problems):
+    """Two independent codes (numpy column sweep in cg_inputs, C loop in the oracle)."""
+    for cfg in (0, 2):
+        p = problems(cfg)
+        y = orc.spmv(p.rowptr, p.colind, p.vals, p.xstar)
+        assert np.all(np.abs(y - p.b) <= 1e-14 * orc.absrow(p.rowptr, p.colind, p.vals, p.xstar))
+
+
+def _lap_eig(n, a, b, c):
+    lam = 6 - 2 * np.cos(a * np.pi / (n + 1)) - 2 * np.cos(b * np.pi / (n + 1)) - 2 * np.cos(c * np.pi / (n + 1))
+    g = np.arange(1, n + 1)
+    v = np.einsum("k,j,i->kji", np.sin(c * np.pi * g / (n + 1)), np.sin(b * np.pi * g / (n + 1)),
+                  np.sin(a * np.pi * g / (n + 1))).ravel()      # node = x + n y + n^2 z
+    return lam, v
+
+
+def test_laplacian_closed_form_eigenpairs(problems):
+    """Closed-form eigenpairs of the 7-point Dirichlet Laplacian on 64^3 (config 1)."""
+    p = problems(1)
+    n = 64
+    for (a, b, c) in [(1, 1, 1), (64, 64, 64), (3, 17, 40), (64, 1, 2)]:
+        lam, v = _lap_eig(n, a, b, c)
+        Av = orc.spmv(p.rowptr, p.colind, p.vals, v)
+        assert np.max(np.abs(Av - lam * v)) <= 1e-14 * 12 * np.max(np.abs(v))
+    lmin, _ = _lap_eig(n, 1, 1, 1)
+    lmax, _ = _lap_eig(n, 64, 64, 64)
+    assert abs(lmin - 0.0070066390) < 1e-9 and abs(lmax - 11.9929933610) < 1e-9
+
+
+def test_dot_series_and_long_double():
+    n = 100003
+    assert orc.dot(np.ones(n), np.ones(n)) == float(n)
+    i = np.arange(1, 2001, dtype=np.float64)
+    assert orc.dot(i, i) == 2000 * 2001 * 4001 / 6            # sum of squares, exact in fp64
+    a, b = gi.seeded_vector(11, n), gi.seeded_vector(12, n)
+    ref = orc.dot_ld(a, b)
+    assert abs(orc.dot(a, b) - ref) <= 1e-15 * np.sum(np.abs(a * b)) * np.log2(n)
+    assert abs(ref - float(np.sum(a.astype(np.longdouble) * b.astype(np.longdouble)))) <= 1e-15 * np.sum(np.abs(a * b))
+
+
+# ---------------------------------------------------------------- CG
+
+def test_cg_handworked_2x2():
+    """tests/golden/cg_2x2_handworked.txt: exact rationals from the textbook recurrences."""
+    g = _golden("cg_2x2_handworked.txt")
+    rp = np.array([0, 2, 4], dtype=np.int32)
+    ci = np.array([0, 1, 0, 1], dtype=np.int32)
+    va = np.array([2.0, -1.0, -1.0, 2.0])
+    r = orc.cg(rp, ci, va, np.array([1.0, 0.0]), rtol=1e-14, maxit=10, keep=3)
+    assert r.iters == int(g["iters"][0]) and r.status == 0
+    np.testing.assert_allclose(r.hist, g["hist"], rtol=0, atol=1e-16)
+    np.testing.assert_allclose(r.alpha, g["alpha"], rtol=1e-15)
+    np.testing.assert_allclose(r.beta[:1], g["beta"], rtol=1e-15)
+    np.testing.assert_allclose(r.x, g["x"], rtol=1e-15)
+    np.testing.assert_allclose(r.P[1], g["p1"], rtol=1e-15)
+
+
+def test_cg_finite_termination_2cubed():
+    """Spectrum {3,5,5,5,7,7,7,9} (tests/golden): four distinct eigenvalues => <= 4 iterations."""
+    g = _golden("laplacian7_2cubed_spectrum.txt")
+    rp, ci, va = gi.laplacian7(2)
+    np.testing.assert_allclose(np.linalg.eigvalsh(_dense(rp, ci, va)), g["eigenvalues"], atol=1e-13)
+    b = gi.seeded_vector(21, 8)
+    r = orc.cg(rp, ci, va, b, rtol=1e-14, maxit=8)
+    assert r.iters <= 4 and r.status == 0
+    assert r.hist[-1] <= 1e-14 * np.linalg.norm(b)
+    np.testing.assert_allclose(r.x, np.linalg.solve(_dense(rp, ci, va), b), rtol=1e-13)
+
+
+def test_cg_finite_termination_three_eigenvectors(problems):
+    """b = sum of 3 eigenvectors of config 1 => 3 iterations, x = sum v/lambda."""
+    p = problems(1)
+    pairs = [_lap_eig(64, *abc) for abc in [(1, 2, 3), (10, 20, 30), (64, 5, 33)]]
+    b = sum(v for _, v in pairs)
+    xs = sum(v / lam for lam, v in pairs)
+    r = orc.cg(p.rowptr, p.colind, p.vals, b, rtol=1e-12, maxit=10)
+    assert r.iters == 3 and r.status == 0
+    assert r.hist[3] / np.linalg.norm(b) < 1e-12
+    assert np.linalg.norm(r.x - xs) / np.linalg.norm(xs) < 1e-13
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_cg_one_step_on_eigenvector(problems, cfg):
+    """b = 0.01*1 is an eigenvector (A*1 = 0.01*1) => one iteration, x = 1."""
+    p = problems(cfg)
+    r = orc.cg(p.rowptr, p.colind, p.vals, np.full(p.n, 0.01), rtol=1e-10, maxit=5)
+    assert r.iters == 1 and r.status == 0
+    assert np.max(np.abs(r.x - 1.0)) < 1e-11
+
+
+def test_cg_vs_dense_cholesky():
+    """Direct solve on 8^3 27-pt (N = 512): catches any wrong sign/scalar in the recurrences."""
+    rp, ci, va = gi.stencil27(8)
+    A = _dense(rp, ci, va)
+    b = gi.seeded_vector(31, 512)
+    L = np.linalg.cholesky(A)
+    xc = np.linalg.solve(L.T, np.linalg.solve(L, b))
+    r = orc.cg(rp, ci, va, b, rtol=1e-12, maxit=512)
+    assert r.status == 0 and 30 <= r.iters <= 120
+    assert np.linalg.norm(r.x - xc) / np.linalg.norm(xc) < 1e-11
+    # nonzero x0 must give the same solution and use r0 = b - A x0
+    x0 = gi.seeded_vector(32, 512)
+    r2 = orc.cg(rp, ci, va, b, x0=x0, rtol=1e-12, maxit=512)
+    assert abs(r2.hist[0] - np.linalg.norm(b - A @ x0)) < 1e-12 * np.linalg.norm(b)
+    assert np.linalg.norm(r2.x - xc) / np.linalg.norm(xc) < 1e-11
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_cg_recovers_known_solution(problems, cfg):
+    p = problems(cfg)
+    r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+    assert r.status == 0
+    assert np.linalg.norm(r.x - p.xstar) / np.linalg.norm(p.xstar) < 1e-7
+    assert r.hist[-1] <= p.rtol * np.linalg.norm(p.b) < r.hist[-2]        # stops at the first crossing
+    assert len(r.hist) == r.iters + 1                                     # reading 6/11
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_recurrence_residual_matches_true_residual(problems, cfg):
+    """Invariant: recurrence r_k equals b - A x_k up to rounding."""
+    p = problems(cfg)
+    r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+    true_r = p.b - orc.spmv_ld(p.rowptr, p.colind, p.vals, r.x)
+    nb = np.linalg.norm(p.b)
+    assert abs(np.linalg.norm(true_r) - r.hist[-1]) / nb < 1e-12
+    assert np.linalg.norm(true_r) / nb <= 2 * p.rtol
+
+
+def test_search_directions_are_A_orthogonal(problems):
+    """p_i^T A p_j ~ 0 and r_i^T r_j ~ 0 (locally, in floating point) on config 0."""
+    p = problems(0)
+    keep = 40
+    r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit, keep=keep)
+    P, R = r.P, r.R
+    AP = np.stack([orc.spmv(p.rowptr, p.colind, p.vals, v) for v in P])
+    G = P @ AP.T
+    d = np.sqrt(np.diag(G))
+    Gn = np.abs(G) / np.outer(d, d)
+    Rn = np.abs(R @ R.T) / np.outer(np.linalg.norm(R, axis=1), np.linalg.norm(R, axis=1))
+    k = len(P)
+    adj = [Gn[i, i + 1] for i in range(k - 1)]
+    assert max(adj) < 1e-12 and max(Rn[i, i + 1] for i in range(k - 1)) < 1e-12
+    win = [Gn[i, j] for i in range(30) for j in range(i + 1, min(i + 11, k))]
+    assert max(win) < 1e-10
+    off = Gn[np.triu_indices(k, 1)]
+    assert off.max() < 1e-8 and Rn[np.triu_indices(k, 1)].max() < 1e-8
+    # p_0 = r_0 and p_{k+1} = r_{k+1} + beta_k p_k (catches a swapped r/p in the update)
+    assert np.array_equal(P[0], R[0])
+    np.testing.assert_allclose(P[5], R[5] + r.beta[4] * P[4], rtol=1e-15, atol=0)
+
+
+def test_lanczos_ritz_values(problems):
+    """alpha/beta sequence => Lanczos T_k; its extreme Ritz values converge to the closed-form
+    lambda_min / lambda_max of config 1 and all lie inside the spectrum."""
+    p = problems(1)
+    r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+    a, b = r.alpha, r.beta
+    k = len(a)
+    d = 1.0 / a
+    d[1:] += b[:-1] / a[:-1]
+    e = np.sqrt(b[:-1]) / a[:-1]
+    T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+    ritz = np.linalg.eigvalsh(T)
+    lmin, lmax = 0.0070066390, 11.9929933610
+    assert ritz.min() >= lmin - 1e-9 and ritz.max() <= lmax + 1e-9
+    assert abs(ritz.min() - lmin) < 1e-6 and abs(ritz.max() - lmax) < 1e-4
+    assert 150 < k < 400
+
+
+def test_convergence_bound_and_monotone_A_norm(problems):
+    """||e_k||_A <= 2 ((sqrt(kappa)-1)/(sqrt(kappa)+1))^k ||e_0||_A, and ||e_k||_A decreases."""
+    p = problems(1)
+    xs = gi.seeded_vector(41, p.n)
+    b = orc.spmv(p.rowptr, p.colind, p.vals, xs)
+    keep = 120
+    r = orc.cg(p.rowptr, p.colind, p.vals, b, rtol=1e-8, maxit=5000, keep=keep)
+    kappa = 11.9929933610 / 0.0070066390
+    rho = (np.sqrt(kappa) - 1) / (np.sqrt(kappa) + 1)
+    eA = []
+    for xk in r.X:
+        e = xk - xs
+        eA.append(np.sqrt(orc.dot(e, orc.spmv(p.rowptr, p.colind, p.vals, e))))
+    eA = np.array(eA)
+    assert np.all(np.diff(eA) < 0)
+    assert np.all(eA <= 2 * rho ** np.arange(len(eA)) * eA[0] * (1 + 1e-12))
+
+
+def test_A_norm_monotone_on_weighted_stencil(problems):
+    p = problems(0)
+    r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit, keep=60)
+    eA = []
+    for xk in r.X:
+        e = xk - p.xstar
+        eA.append(orc.dot(e, orc.spmv(p.rowptr, p.colind, p.vals, e)))
+    assert np.all(np.diff(np.array(eA)) < 0)
+
+
+# ---------------------------------------------------------------- conventions (DESIGN.md readings)
+
+def test_conventions_zero_rhs_maxit_breakdown_x0():
+    rp, ci, va = gi.stencil27(4)
+    n = 64
+    r = orc.cg(rp, ci, va, np.zeros(n), x0=np.ones(n), rtol=1e-10, maxit=10)
+    assert r.iters == 0 and r.status == 0 and np.all(r.x == 0) and r.hist.tolist() == [0.0]   # reading 9
+    b = gi.seeded_vector(51, n)
+    r = orc.cg(rp, ci, va, b, rtol=0.0, maxit=7)
+    assert r.iters == 7 and r.status == 1 and len(r.hist) == 8                                  # reading 7
+    r = orc.cg(rp, ci, va, b, rtol=1e-10, maxit=0)
+    assert r.iters == 0 and r.status == 1
+    A = _dense(rp, ci, va)
+    xs = np.linalg.solve(A, b)
+    r = orc.cg(rp, ci, va, b, x0=xs, rtol=1e-10, maxit=10)
+    assert r.iters == 0 and r.status == 0                                                       # reading 5
+    r = orc.cg(rp, ci, -va, b, rtol=1e-10, maxit=10)                                            # -A: not SPD
+    assert r.status == 2 and r.iters == 0
+
+
+def test_jacobi_pcg_matches_cg_on_scaled_system():
+    """PCG with M = D equals plain CG on D^-1/2 A D^-1/2 (textbook identity): pins the
+    preconditioned branch used by the 8(f) rank-1 row."""
+    p = gi.make_config(4, grid=12)
+    A = _dense(p.rowptr, p.colind, p.vals)
+    d = np.diag(A)
+    r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=1e-10, maxit=2000, dinv=1.0 / d)
+    assert r.status == 0
+    xd = np.linalg.solve(A, p.b)
+    assert np.linalg.norm(r.x - xd) / np.linalg.norm(xd) < 1e-8
+    s = 1.0 / np.sqrt(d)
+    va2 = p.vals * s[np.repeat(np.arange(p.n), np.diff(p.rowptr))] * s[p.colind]
+    r2 = orc.cg(p.rowptr, p.colind, va2, s * p.b, rtol=0.0, maxit=20)
+    r1 = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=0.0, maxit=20, dinv=1.0 / d)
+    np.testing.assert_allclose(r1.alpha, r2.alpha, rtol=1e-9)
+    np.testing.assert_allclose(r1.beta, r2.beta, rtol=1e-9)
+    plain = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=1e-10, maxit=20000)
+    assert r.iters < plain.iters
+
+
+def test_iteration_counts_reported_not_pinned(problems):
+    """Parity unpinned (oracle header): nothing external fixes these counts.  They are only
+    sanity-bounded here so a gross regression is seen."""
+    lo_hi = {0: (50, 200), 1: (150, 400), 2: (100, 450), 3: (100, 500)}
+    for cfg, (lo, hi) in lo_hi.items():
+        p = problems(cfg)
+        r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+        assert r.status == 0 and lo <= r.iters <= hi, (cfg, r.iters)
