@@ -1,0 +1,140 @@
+/*
+ * cg.h -- C ABI of libcg_b200: fp64 conjugate gradient on a CSR SPD matrix,
+ * hand-written CUDA for sm_100a (one B200, no sharding, no collectives).
+ *
+ * The operation is the case study of arxiv 1107.0538 ("The conjugate
+ * gradient (CG) method ... The matrix is stored in Compressed Sparse Row (CSR)
+ * format having N=132651 and NNZ=3442951"; "DGEMV(sparse)", the CGLoop
+ * with its continue-condition; PAPER.md:48 double precision; PAPER.md:60 TOL=1E-10).
+ * Unlike the paper, which runs "scalar operations ... on CPU processor"
+ * and loses its multi-GPU speed-up to "extra data transfers among cpu and devices"
+ * (PAPER.md:50), alpha, beta and the stop test stay on the device: cg_solve makes
+ * exactly one host synchronisation, at the end.
+ *
+ * Conventions:
+ *  - d_* pointers are DEVICE memory owned by the caller (e.g. torch tensors),
+ *    16-byte aligned; h_* pointers are HOST memory.  `cuda_stream` is a
+ *    cudaStream_t passed as void* (0 = the legacy default stream).
+ *  - The handle BORROWS rowptr/colind/vals and the workspace: they must outlive
+ *    it and must not be written while a call is in flight.  The library never
+ *    allocates or frees device memory (only the small host struct, 64 bytes of
+ *    pinned host memory and, in graph mode, a CUDA graph).
+ *  - CSR: 0-based int32 indices, rowptr[0] = 0, rowptr[n] = nnz, non-decreasing.
+ *    Columns of a row need not be sorted or unique (duplicates add).
+ *  - Return codes: 0 success / converged.  Positive = soft outcome of cg_solve:
+ *    1 maxit reached, 2 breakdown (p.Ap <= 0 or not finite: A is not SPD).
+ *    Negative = error: -1 invalid argument, -2 CUDA error (text via
+ *    cg_strerror), -3 device not supported (needs compute capability 10.x).
+ *    Nothing is printed, thrown or aborted across this boundary.
+ *  - One handle per stream; concurrent calls on one handle are undefined.
+ */
+#ifndef CG_B200_H
+#define CG_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cg_handle cg_handle;
+
+#define CG_OK             0
+#define CG_MAXIT          1
+#define CG_BREAKDOWN      2
+#define CG_EINVAL        -1
+#define CG_ECUDA         -2
+#define CG_EUNSUPPORTED  -3
+
+/* Bytes of device workspace cg_create needs for an n-row system: the vectors
+ * r, p, p', q, z, D^-1 (each n doubles, 256-byte aligned), the per-CTA reduction
+ * partials, the device-resident scalar state and the grid-barrier word. */
+size_t cg_workspace_bytes(int64_t n);
+
+/* Bind a handle to a CSR matrix already resident on the device.
+ * d_rowptr int32[n+1], d_colind int32[nnz], d_vals double[nnz].
+ * d_workspace: >= cg_workspace_bytes(n) bytes, 256-byte aligned.
+ * Reads n+1 row pointers once (one stream-0 kernel) to pick the SpMV tiling.
+ * Errors: CG_EINVAL on NULL/misaligned pointers, n <= 0, nnz < 0, n or nnz
+ * >= 2^31, workspace too small; CG_EUNSUPPORTED off sm_100; CG_ECUDA. */
+int cg_create(cg_handle** out, int64_t n, int64_t nnz,
+              const int32_t* d_rowptr, const int32_t* d_colind, const double* d_vals,
+              void* d_workspace, size_t workspace_bytes);
+
+/* Optional structural check of the bound CSR arrays on the device: rowptr[0] = 0,
+ * rowptr[n] = nnz, non-decreasing, 0 <= colind < n.  Synchronises the stream.
+ * Returns CG_OK or CG_EINVAL.  (Symmetry / definiteness are NOT checked:
+ * PAPER.md:34 "should only be applied to" SPD systems; cg_solve reports
+ * CG_BREAKDOWN instead.) */
+int cg_check_csr(cg_handle* h, void* cuda_stream);
+
+/* y = A x, the paper's "DGEMV(sparse)".  d_x, d_y: double[n],
+ * distinct buffers.  Asynchronous on the stream. */
+int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_stream);
+
+/* *h_result = sum_i a_i b_i (the p.Ap / r.r reductions of the CG loop), with a
+ * fixed reduction order: bitwise reproducible run to run.  d_a, d_b: double[n].
+ * Synchronises the stream once. */
+int cg_dot(cg_handle* h, const double* d_a, const double* d_b,
+           double* h_result, void* cuda_stream);
+
+/* Solve A x = b by unpreconditioned CG (readings in DESIGN.md):
+ *   r = b - A x0; p = r; loop { q = A p; alpha = r.r / p.q; x += alpha p;
+ *   r -= alpha q; beta = r'.r' / r.r; p = r + beta p } until
+ *   ||r_k||_2 <= rtol ||b||_2 (tested before the first iteration and after
+ *   every update) or k = maxit (the paper's CGLoop bound is N).
+ * d_b double[n] (not modified); d_x double[n]: x0 on entry, x_k on return.
+ * d_hist: device double[maxit+1] or NULL; d_hist[j] = ||r_j||_2 for j = 0..k.
+ * *h_iters = k (number of in-loop SpMVs); *h_final_resnorm = ||r_k||_2.
+ * b = 0 returns x = 0, k = 0, CG_OK.  Synchronises the stream once, at the end.
+ * Returns CG_OK / CG_MAXIT / CG_BREAKDOWN or a negative error. */
+int cg_solve(cg_handle* h, const double* d_b, double* d_x,
+             double rtol, int64_t maxit, double* d_hist,
+             int64_t* h_iters, double* h_final_resnorm, void* cuda_stream);
+
+/* Jacobi-preconditioned variant (the paper's sequential
+ * reference is Matlab's *p*cg): z = D^-1 r with D = diag(A) taken
+ * from the CSR arrays; alpha = r.z / p.q, beta = r'.z' / r.z, p = z + beta p.
+ * The stop test is still on ||r_k||_2.  Same arguments and returns as cg_solve;
+ * CG_BREAKDOWN also when a diagonal entry is missing or not positive. */
+int cg_solve_jacobi(cg_handle* h, const double* d_b, double* d_x,
+                    double rtol, int64_t maxit, double* d_hist,
+                    int64_t* h_iters, double* h_final_resnorm, void* cuda_stream);
+
+/* End-to-end entry with HOST buffers: copies h_b and h_x (x0) to the device,
+ * runs cg_solve, copies x and hist[0..k] back.  h_b, h_x double[n]; h_hist
+ * double[maxit+1] or NULL.  d_scratch: device memory of at least
+ * cg_host_scratch_bytes(n, maxit) bytes, 256-byte aligned.  Pinned host
+ * buffers make the copies asynchronous; pageable ones also work. */
+size_t cg_host_scratch_bytes(int64_t n, int64_t maxit);
+int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
+                  double rtol, int64_t maxit, double* h_hist,
+                  int64_t* h_iters, double* h_final_resnorm,
+                  void* d_scratch, size_t scratch_bytes, void* cuda_stream);
+
+/* Tuning / diagnostics.  Options (name -> value):
+ *   "loop"  0 = one cooperative persistent kernel (default)
+ *           1 = CUDA graph of {K1, K2, K3} per iteration, replayed in chunks
+ *               with a device-side stop flag (the profilable twin)
+ *           2 = plain per-iteration launches, same kernels as 1
+ *   "spmv"  0 = auto, 1 = sub-warp-per-row from global memory,
+ *           2 = bulk-async (TMA) streamed tiles, thread per row
+ *   "chunk" iterations per graph replay in loop mode 1 (even, default 32)
+ * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches"
+ * (kernels launched by the last call), "sms".
+ * Unknown names return CG_EINVAL. */
+int cg_set_option(cg_handle* h, const char* name, int64_t value);
+int cg_get_info(cg_handle* h, const char* name, int64_t* value);
+
+/* Frees the host struct (and any CUDA graph).  Device memory is the caller's. */
+int cg_destroy(cg_handle* h);
+
+/* Static text for a return code; for CG_ECUDA the last CUDA error string seen
+ * by this thread. */
+const char* cg_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CG_B200_H */

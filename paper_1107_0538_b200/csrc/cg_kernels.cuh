@@ -1,0 +1,464 @@
+// cg_kernels.cuh -- device code of the fp64 CSR conjugate-gradient hot path for sm_100a.
+//
+// Steps (the paper names only the first, PAPER.md:44
+// "Tasks, such as DGEMV(sparse), are repetitive"; the rest is the textbook CG of
+// its ref [5]):
+//   K1  q = A p fused with the p.q partial sums           (phase_spmv_*)
+//   K2  x += alpha p ; r -= alpha q ; partial sums of r.r (phase_update_xr)
+//   K3  p = r + beta p                                    (phase_update_p)
+// alpha, beta and the continue-condition are evaluated on the
+// device, redundantly and identically by every CTA, from per-CTA partials summed
+// in a fixed order -- the paper's CPU-side scalar step and its transfers
+// do not exist here.
+//
+// The same phase functions are used by the persistent cooperative kernel and by
+// the three stand-alone kernels of the graph / stepwise loop, so all loop modes
+// give bitwise identical results for equal grid and block sizes.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cgk {
+
+constexpr int kThreads = 256;       // threads per CTA, every kernel
+constexpr int kWarps = kThreads / 32;
+constexpr int kMaxGrid = 2048;      // capacity of each partials array
+
+// SpMV variant B (bulk-async streamed tiles): each warp owns a private ring of
+// kStages tiles of kTileRows rows; a tile's nnz span must fit kTileCap entries.
+constexpr int kTileRows = 32;
+constexpr int kTileCap = 1016;      // nnz per tile (<= 31.75 per row on average)
+constexpr int kTileBuf = kTileCap + 8;   // + up to 3 entries of widening at each end, padded
+constexpr int kStages = 2;
+
+struct State {            // one per iteration parity (loop modes 1, 2)
+    double rr;            // ||r_k||^2
+    double rz;            // r_k . z_k (== rr without preconditioner)
+    long long k;          // iterations done
+    int stop;             // 0 run, 1 stop
+    int status;           // CG_OK / CG_MAXIT / CG_BREAKDOWN once stopped
+};
+
+struct Scal {             // device-resident scalar state, zeroed before each solve
+    State st[2];
+    double bb;            // ||b||^2
+    double thresh;        // rtol * ||b||
+    int brk[2];           // breakdown seen by K2 of this parity
+    unsigned long long bar;       // grid barrier arrival counter
+    long long out_iters;  // result block, copied to the host at the end
+    long long out_status;
+    double out_res;
+    double dot_out;       // cg_dot result
+    int check;            // cg_check_csr error bits            (not zeroed per solve from here on)
+    int diag_bad;         // Jacobi: a diagonal entry is missing or not positive
+    int max_row_len;      // cg_create statistics
+    int max_tile_nnz;
+};
+
+struct Params {
+    long long n, nnz;
+    const int* rowptr;
+    const int* colind;
+    const double* vals;
+    const double* b;
+    double* x;
+    double* r;
+    double* p;
+    double* q;
+    double* dinv;
+    double* part0;        // p.q
+    double* part1;        // r.r
+    double* part2;        // r.z (Jacobi) ; b.b in the prologue
+    double* part3;        // r0.z0 in the prologue (Jacobi)
+    Scal* scal;
+    double* hist;         // may be null
+    double rtol;
+    long long maxit;
+    int precond;          // 0 none (the paper's path), 1 Jacobi
+    int spmv;             // 1 vector, 2 stream
+    int tpr;              // lanes per row of the vector variant
+};
+
+// ---------------------------------------------------------------- small helpers
+
+__device__ __forceinline__ double ld_stream_f64(const double* p) {
+    double v;   // matrix values are read once per SpMV: read-only path, do not allocate in L1
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int ld_stream_s32(const int* p) {
+    int v;
+    asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_add_u64(unsigned long long* p, unsigned long long v) {
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum of one value per thread over the CTA, fixed order.  Result valid in thread 0.
+__device__ __forceinline__ double block_sum(double v, double* sm) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = warp_sum(v);
+    __syncthreads();                       // sm may still be read from a previous call
+    if (lane == 0) sm[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = lane < kWarps ? sm[lane] : 0.0;
+        v = warp_sum(v);
+    }
+    return v;
+}
+
+// Fixed-order sum of the G per-CTA partials; every thread of the CTA gets the value.
+__device__ __forceinline__ double sum_partials(const double* part, int G, double* sm) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (warp == 0) {
+        double s = 0.0;
+        for (int j = lane; j < G; j += 32) s += __ldcg(part + j);
+        s = warp_sum(s);
+        if (lane == 0) sm[kWarps] = s;
+    }
+    __syncthreads();
+    return sm[kWarps];
+}
+
+// Grid-wide barrier for the cooperative persistent kernel (all CTAs co-resident).
+// One arrival counter, never reset inside a solve; `epoch` is the local target.
+__device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned int G,
+                                             unsigned long long& epoch) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        epoch += G;
+        __threadfence();
+        red_release_add_u64(bar, 1ULL);
+        while (ld_acquire_u64(bar) < epoch) { }
+        __threadfence();                   // also invalidates this SM's L1 (CCTL.IVALL)
+    }
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------- K1, variant A
+// Sub-warp of TPR lanes per row, straight from global memory.  Generic fallback:
+// any CSR matrix, any row length.
+template <int TPR, bool DOT>
+__device__ __forceinline__ double phase_spmv_vector(const Params& P, const double* x, double* y,
+                                                    int cta, int G) {
+    const int* __restrict__ rowptr = P.rowptr;
+    const int* __restrict__ colind = P.colind;
+    const double* __restrict__ vals = P.vals;
+    constexpr int kRows = kThreads / TPR;
+    const int lir = threadIdx.x % TPR;
+    const int sub = threadIdx.x / TPR;
+    double dot = 0.0;
+    for (long long row0 = (long long)cta * kRows; row0 < P.n; row0 += (long long)G * kRows) {
+        const long long row = row0 + sub;
+        double acc = 0.0;
+        if (row < P.n) {
+            const int s = __ldg(rowptr + row), e = __ldg(rowptr + row + 1);
+            for (int k = s + lir; k < e; k += 4 * TPR) {
+                const int k1 = k + TPR, k2 = k + 2 * TPR, k3 = k + 3 * TPR;
+                const bool b1 = k1 < e, b2 = k2 < e, b3 = k3 < e;
+                const int c0 = ld_stream_s32(colind + k);
+                const int c1 = b1 ? ld_stream_s32(colind + k1) : c0;
+                const int c2 = b2 ? ld_stream_s32(colind + k2) : c0;
+                const int c3 = b3 ? ld_stream_s32(colind + k3) : c0;
+                const double v0 = ld_stream_f64(vals + k);
+                const double v1 = b1 ? ld_stream_f64(vals + k1) : 0.0;
+                const double v2 = b2 ? ld_stream_f64(vals + k2) : 0.0;
+                const double v3 = b3 ? ld_stream_f64(vals + k3) : 0.0;
+                const double x0 = x[c0], x1 = x[c1], x2 = x[c2], x3 = x[c3];
+                acc = fma(v0, x0, acc);
+                acc = fma(v1, x1, acc);
+                acc = fma(v2, x2, acc);
+                acc = fma(v3, x3, acc);
+            }
+        }
+#pragma unroll
+        for (int o = TPR / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (row < P.n && lir == 0) {
+            y[row] = acc;
+            if (DOT) dot = fma(acc, x[row], dot);
+        }
+    }
+    return dot;
+}
+
+template <bool DOT>
+__device__ __forceinline__ double phase_spmv_vector_dispatch(const Params& P, const double* x,
+                                                             double* y, int cta, int G) {
+    switch (P.tpr) {
+        case 2:  return phase_spmv_vector<2, DOT>(P, x, y, cta, G);
+        case 4:  return phase_spmv_vector<4, DOT>(P, x, y, cta, G);
+        case 8:  return phase_spmv_vector<8, DOT>(P, x, y, cta, G);
+        case 16: return phase_spmv_vector<16, DOT>(P, x, y, cta, G);
+        default: return phase_spmv_vector<32, DOT>(P, x, y, cta, G);
+    }
+}
+
+// ---------------------------------------------------------------- K1, variant B
+// Bulk-async (TMA, cp.async.bulk -> SASS UBLKCP) streaming of the contiguous
+// vals/colind span of a 32-row tile into a warp-private shared-memory ring, then
+// one thread per row walks its entries out of shared memory.  For the natural-
+// ordered stencil the x gathers of the 32 lanes are consecutive addresses.
+//
+// Alignment: cp.async.bulk needs 16-byte aligned source, destination and size.
+// The span [s, e) of a tile is widened to [s & ~3, ...) so both the int32 and the
+// fp64 source addresses are 16-byte aligned (the arrays themselves are, by the
+// cg_create contract); the end is rounded up but clamped to nnz rounded DOWN to a
+// multiple of 4, and the <= 3 trailing entries of the whole matrix are fetched
+// with ordinary loads, so nothing outside the arrays is ever touched.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
+                 :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) { }
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar,
+                                         uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1], %2, [%3], %4;"
+        :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
+struct __align__(16) WarpStage {
+    double vals[kTileBuf];
+    int cols[kTileBuf];
+};
+struct StreamSmem {
+    WarpStage stage[kWarps][kStages];
+    uint64_t full[kWarps][kStages];
+};
+constexpr size_t kStreamSmemBytes = sizeof(StreamSmem);
+
+// Issue the copies for tile `t` into `st` (called by lane 0 of the owning warp).
+// Returns nothing; the span base (first fetched entry index) is recomputed by readers.
+__device__ __forceinline__ void stream_issue(const Params& P, long long t, WarpStage* st,
+                                             uint64_t* bar, uint64_t policy) {
+    const long long row0 = t * kTileRows;
+    const long long row1 = (row0 + kTileRows < P.n) ? row0 + kTileRows : P.n;
+    const int s = __ldg(P.rowptr + row0), e = __ldg(P.rowptr + row1);
+    const int s4 = s & ~3;
+    const int lim = (int)(P.nnz & ~3LL);              // last entry reachable by bulk copies
+    int e4 = (e + 3) & ~3;
+    if (e4 > lim) e4 = lim;
+    const int cnt = e4 > s4 ? e4 - s4 : 0;            // multiple of 4
+    if (cnt > 0) {
+        mbar_expect_tx(bar, (uint32_t)cnt * 12u);
+        bulk_g2s(st->vals, P.vals + s4, (uint32_t)cnt * 8u, bar, policy);
+        bulk_g2s(st->cols, P.colind + s4, (uint32_t)cnt * 4u, bar, policy);
+    } else {
+        mbar_expect_tx(bar, 0u);
+    }
+}
+
+template <bool DOT>
+__device__ __forceinline__ double phase_spmv_stream(const Params& P, const double* x, double* y,
+                                                    int cta, int G, StreamSmem* sm,
+                                                    uint32_t& phase_bits) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long ntiles = (P.n + kTileRows - 1) / kTileRows;
+    const long long gw = (long long)cta * kWarps + warp;          // global warp id
+    const long long nw = (long long)G * kWarps;
+    const uint64_t policy = l2_policy_evict_first();
+    const int lim = (int)(P.nnz & ~3LL);
+    double dot = 0.0;
+
+    // prime the ring
+    if (lane == 0) {
+#pragma unroll
+        for (int sidx = 0; sidx < kStages; ++sidx) {
+            const long long t = gw + (long long)sidx * nw;
+            if (t < ntiles) stream_issue(P, t, &sm->stage[warp][sidx], &sm->full[warp][sidx], policy);
+        }
+    }
+    int sidx = 0;
+    for (long long t = gw; t < ntiles; t += nw) {
+        WarpStage* st = &sm->stage[warp][sidx];
+        const long long row = t * kTileRows + lane;
+        const long long rlast = (t * kTileRows + kTileRows < P.n) ? t * kTileRows + kTileRows : P.n;
+        const int tile_s = __ldg(P.rowptr + t * kTileRows);
+        const int tile_e = __ldg(P.rowptr + rlast);
+        const int base = tile_s & ~3;
+        int s = 0, e = 0;
+        if (row < P.n) { s = __ldg(P.rowptr + row); e = __ldg(P.rowptr + row + 1); }
+        // trailing <= 3 entries of the matrix that no bulk copy may cover
+        if (tile_e > lim) {
+            const int k = lim + lane;
+            if (lane < 4 && k < tile_e && k >= base) {
+                st->vals[k - base] = ld_stream_f64(P.vals + k);
+                st->cols[k - base] = ld_stream_s32(P.colind + k);
+            }
+        }
+        mbar_wait(&sm->full[warp][sidx], (phase_bits >> sidx) & 1u);
+        phase_bits ^= (1u << sidx);
+        __syncwarp();
+        double acc = 0.0;
+        for (int k = s - base; k < e - base; ++k)
+            acc = fma(st->vals[k], x[st->cols[k]], acc);
+        if (row < P.n) {
+            y[row] = acc;
+            if (DOT) dot = fma(acc, x[row], dot);
+        }
+        __syncwarp();                      // every lane is done reading this stage
+        const long long tn = t + (long long)kStages * nw;
+        if (lane == 0 && tn < ntiles)
+            stream_issue(P, tn, st, &sm->full[warp][sidx], policy);
+        sidx = (sidx + 1 == kStages) ? 0 : sidx + 1;
+    }
+    return dot;
+}
+
+// ---------------------------------------------------------------- vector phases
+
+// Prologue: r = b - q (q = A x0); p = r (or D^-1 r); partials of r.r, b.b, r.z.
+__device__ __forceinline__ void phase_init_residual(const Params& P, int cta, int G, double* sm) {
+    const double* __restrict__ b = P.b;
+    const double* __restrict__ q = P.q;
+    const double* __restrict__ dinv = P.dinv;
+    double* __restrict__ r = P.r;
+    double* __restrict__ p = P.p;
+    double arr = 0.0, abb = 0.0, arz = 0.0;
+    const long long stride = (long long)G * kThreads;
+    for (long long i = (long long)cta * kThreads + threadIdx.x; i < P.n; i += stride) {
+        const double bi = b[i];
+        const double ri = bi - q[i];
+        r[i] = ri;
+        abb = fma(bi, bi, abb);
+        arr = fma(ri, ri, arr);
+        if (P.precond) {
+            const double zi = dinv[i] * ri;
+            p[i] = zi;
+            arz = fma(ri, zi, arz);
+        } else {
+            p[i] = ri;
+        }
+    }
+    double t = block_sum(arr, sm); if (threadIdx.x == 0) P.part1[cta] = t;
+    t = block_sum(abb, sm);        if (threadIdx.x == 0) P.part2[cta] = t;
+    if (P.precond) { t = block_sum(arz, sm); if (threadIdx.x == 0) P.part3[cta] = t; }
+}
+
+// K2: x += alpha p ; r -= alpha q ; partial r.r (and r.z with Jacobi).
+__device__ __forceinline__ void phase_update_xr(const Params& P, double alpha, int cta, int G,
+                                                double* sm) {
+    const double na = -alpha;
+    double arr = 0.0, arz = 0.0;
+    const long long np2 = P.n >> 1;
+    const long long stride = (long long)G * kThreads;
+    double2* __restrict__ x2 = reinterpret_cast<double2*>(P.x);
+    double2* __restrict__ r2 = reinterpret_cast<double2*>(P.r);
+    const double2* __restrict__ p2 = reinterpret_cast<const double2*>(P.p);
+    const double2* __restrict__ q2 = reinterpret_cast<const double2*>(P.q);
+    const double2* __restrict__ d2 = reinterpret_cast<const double2*>(P.dinv);
+#pragma unroll 2
+    for (long long i = (long long)cta * kThreads + threadIdx.x; i < np2; i += stride) {
+        double2 xv = x2[i], rv = r2[i];
+        const double2 pv = p2[i], qv = q2[i];
+        xv.x = fma(alpha, pv.x, xv.x); xv.y = fma(alpha, pv.y, xv.y);
+        rv.x = fma(na, qv.x, rv.x);    rv.y = fma(na, qv.y, rv.y);
+        x2[i] = xv; r2[i] = rv;
+        arr = fma(rv.x, rv.x, arr); arr = fma(rv.y, rv.y, arr);
+        if (P.precond) {
+            const double2 dv = d2[i];
+            arz = fma(rv.x, dv.x * rv.x, arz); arz = fma(rv.y, dv.y * rv.y, arz);
+        }
+    }
+    if ((P.n & 1) && cta == G - 1 && threadIdx.x == kThreads - 1) {      // odd tail element
+        const long long i = P.n - 1;
+        const double xi = fma(alpha, P.p[i], P.x[i]);
+        const double ri = fma(na, P.q[i], P.r[i]);
+        P.x[i] = xi; P.r[i] = ri;
+        arr = fma(ri, ri, arr);
+        if (P.precond) arz = fma(ri, P.dinv[i] * ri, arz);
+    }
+    double t = block_sum(arr, sm); if (threadIdx.x == 0) P.part1[cta] = t;
+    if (P.precond) { t = block_sum(arz, sm); if (threadIdx.x == 0) P.part2[cta] = t; }
+}
+
+// K3: p = r + beta p   (Jacobi: p = D^-1 r + beta p).
+__device__ __forceinline__ void phase_update_p(const Params& P, double beta, int cta, int G) {
+    const long long np2 = P.n >> 1;
+    const long long stride = (long long)G * kThreads;
+    double2* __restrict__ p2 = reinterpret_cast<double2*>(P.p);
+    const double2* __restrict__ r2 = reinterpret_cast<const double2*>(P.r);
+    const double2* __restrict__ d2 = reinterpret_cast<const double2*>(P.dinv);
+#pragma unroll 2
+    for (long long i = (long long)cta * kThreads + threadIdx.x; i < np2; i += stride) {
+        double2 pv = p2[i];
+        double2 rv = r2[i];
+        if (P.precond) { const double2 dv = d2[i]; rv.x *= dv.x; rv.y *= dv.y; }
+        pv.x = fma(beta, pv.x, rv.x); pv.y = fma(beta, pv.y, rv.y);
+        p2[i] = pv;
+    }
+    if ((P.n & 1) && cta == G - 1 && threadIdx.x == kThreads - 1) {
+        const long long i = P.n - 1;
+        double ri = P.r[i];
+        if (P.precond) ri *= P.dinv[i];
+        P.p[i] = fma(beta, P.p[i], ri);
+    }
+}
+
+// x = 0 (the b = 0 convention)
+__device__ __forceinline__ void phase_zero_x(const Params& P, int cta, int G) {
+    const long long stride = (long long)G * kThreads;
+    for (long long i = (long long)cta * kThreads + threadIdx.x; i < P.n; i += stride) P.x[i] = 0.0;
+}
+
+// One SpMV phase.  VARIANT 1 = sub-warp per row from global, 2 = streamed tiles.
+template <int VARIANT, bool DOT>
+__device__ __forceinline__ double phase_spmv(const Params& P, const double* x, double* y, int cta,
+                                             int G, unsigned char* dyn_smem, uint32_t& phase_bits) {
+    if constexpr (VARIANT == 2)
+        return phase_spmv_stream<DOT>(P, x, y, cta, G, reinterpret_cast<StreamSmem*>(dyn_smem),
+                                      phase_bits);
+    else
+        return phase_spmv_vector_dispatch<DOT>(P, x, y, cta, G);
+}
+
+template <int VARIANT>
+__device__ __forceinline__ void stream_smem_init(unsigned char* dyn_smem) {
+    if constexpr (VARIANT == 2) {
+        StreamSmem* sm = reinterpret_cast<StreamSmem*>(dyn_smem);
+        if (threadIdx.x < kWarps * kStages)
+            mbar_init(&sm->full[threadIdx.x / kStages][threadIdx.x % kStages], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+    }
+}
+
+}  // namespace cgk

@@ -1,0 +1,78 @@
+"""CPU-side checks of the C-ABI boundary: the library builds, loads, and exports every symbol
+include/cg.h declares.  No compute call is made (there is no GPU here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "cg.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(cg_[a-z_]+)\s*\(", src)))
+
+
+def test_header_declares_the_boundary():
+    names = _declared()
+    for must in ("cg_create", "cg_spmv", "cg_dot", "cg_solve", "cg_destroy", "cg_strerror",
+                 "cg_workspace_bytes"):
+        assert must in names
+    text = open(os.path.join(ROOT, "include", "cg.h")).read()
+    assert 'extern "C"' in text and "torch" not in text.replace("torch tensors", "")
+
+
+def test_library_builds_and_exports_every_symbol():
+    from paper_1107_0538_b200 import binding, build
+    path = build.build()
+    assert os.path.exists(path)
+    L = ctypes.CDLL(path)
+    for name in _declared():
+        assert hasattr(L, name), f"{name} declared in include/cg.h but not exported"
+    assert set(_declared()) == set(binding.SIGNATURES), "binding.SIGNATURES out of sync with cg.h"
+
+
+def test_host_only_entry_points():
+    import paper_1107_0538_b200 as cg
+    assert cg.cg_workspace_bytes(0) == 0 and cg.cg_workspace_bytes(-5) == 0
+    n = 132651
+    wb = cg.cg_workspace_bytes(n)
+    assert wb >= 5 * 8 * n and wb % 256 == 0
+    assert cg.cg_host_scratch_bytes(n, n) >= 8 * (3 * n + 1)
+    assert "invalid" in cg.cg_strerror(-1)
+    assert "breakdown" in cg.cg_strerror(2).lower()
+    assert cg.cg_strerror(0) and cg.cg_strerror(1) and cg.cg_strerror(-3)
+    # NULL handles are rejected without touching a device
+    L = cg.lib()
+    assert L.cg_spmv(None, None, None, None) == -1
+    assert L.cg_solve(None, None, None, 1e-10, 10, None, None, None, None) == -1
+    assert L.cg_set_option(None, b"loop", 0) == -1
+    assert L.cg_destroy(None) == 0
+
+
+def test_sass_is_sm100a_with_bulk_async_copies():
+    """The streamed SpMV must really use cp.async.bulk (SASS UBLKCP) and be built for sm_100a."""
+    import shutil
+    import subprocess
+    from paper_1107_0538_b200 import build
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    out = subprocess.run([cuobjdump, "-sass", build.build()], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    assert "UBLKCP" in out
+    assert "DFMA" in out
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1107_0538_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.lower() or f == "__init__.py" and False, f"{f} mentions the oracle"
+    for f in ("cg_oracle.c", "cg_oracle.py"):
+        text = open(os.path.join(ROOT, "oracle", f)).read()
+        assert "paper_1107_0538_b200 import" not in text and "libcg_b200" not in text

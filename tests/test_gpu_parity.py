@@ -1,0 +1,383 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, on the same seeded inputs.
+
+Tolerances are BASELINE.json north_star's, with the readings of SURVEY.md 8(c) 12-15:
+  SpMV        |y_gpu - y_or|_i <= 1e-13 * (|A||x|)_i
+  history     |h_gpu[j] - h_or[j]| / h_or[j] <= 1e-9 for j = 0..min(50, k)
+  iterations  within +-2 % of the oracle's count (at least +-1)
+  solution    ||x_gpu - x_or||_2 / ||x_or||_2 <= 1e-8
+"""
+import math
+
+import numpy as np
+import pytest
+
+import cg_inputs as gi
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+SPMV_TOL = 1e-13
+HIST_TOL = 1e-9
+X_TOL = 1e-8
+
+
+@pytest.fixture(scope="module")
+def cgmod():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device")
+    import paper_1107_0538_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import cg_oracle
+    return cg_oracle
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+class Bound:
+    def __init__(self, m, p):
+        self.p = p
+        self.cg = m.CG(dev(p.rowptr), dev(p.colind), dev(p.vals))
+        self.b = dev(p.b)
+
+
+@pytest.fixture(scope="module")
+def bound(cgmod, problems):
+    cache = {}
+
+    def get(cfg, grid=None):
+        if (cfg, grid) not in cache:
+            cache[(cfg, grid)] = Bound(cgmod, problems(cfg, grid))
+        return cache[(cfg, grid)]
+    yield get
+    for b in cache.values():
+        b.cg.close()
+
+
+_oracle_cache = {}
+
+
+def oracle_solve(orc, p, key, **kw):
+    if key not in _oracle_cache:
+        _oracle_cache[key] = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=kw.get("rtol", p.rtol),
+                                    maxit=kw.get("maxit", p.maxit), dinv=kw.get("dinv"))
+    return _oracle_cache[key]
+
+
+def check_solve_parity(res, x, ref, iters_band=True):
+    k = min(50, ref.iters, res.iters)
+    hg = res.hist.cpu().numpy()
+    rel = np.abs(hg[:k + 1] - ref.hist[:k + 1]) / ref.hist[:k + 1]
+    assert rel.max() <= HIST_TOL, f"history differs: {rel.max():.3e}"
+    if iters_band:
+        band = max(1, math.floor(0.02 * ref.iters))
+        assert abs(res.iters - ref.iters) <= band, (res.iters, ref.iters)
+    xe = np.linalg.norm(x.cpu().numpy() - ref.x) / np.linalg.norm(ref.x)
+    assert xe <= X_TOL, f"solution differs: {xe:.3e}"
+    assert res.status == ref.status
+    assert len(hg) == res.iters + 1
+
+
+# ---------------------------------------------------------------- SpMV / dot
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_spmv_parity(bound, orc, cfg, variant):
+    B = bound(cfg)
+    p = B.p
+    B.cg.set_option("spmv", variant)
+    assert B.cg.info("spmv") == variant
+    x = gi.seeded_vector(100 + cfg, p.n)
+    y = B.cg.spmv(dev(x)).cpu().numpy()
+    want = orc.spmv(p.rowptr, p.colind, p.vals, x)
+    denom = orc.absrow(p.rowptr, p.colind, p.vals, x)
+    err = np.abs(y - want) / denom
+    assert err.max() <= SPMV_TOL, f"cfg {cfg} variant {variant}: {err.max():.3e}"
+    B.cg.set_option("spmv", 0)
+
+
+@pytest.mark.parametrize("tpr", [2, 4, 8, 16, 32])
+def test_spmv_vector_all_lane_widths(bound, orc, tpr):
+    B = bound(0)
+    p = B.p
+    B.cg.set_option("spmv", 1)
+    B.cg.set_option("tpr", tpr)
+    x = gi.seeded_vector(7, p.n)
+    y = B.cg.spmv(dev(x)).cpu().numpy()
+    want = orc.spmv(p.rowptr, p.colind, p.vals, x)
+    assert np.all(np.abs(y - want) <= SPMV_TOL * orc.absrow(p.rowptr, p.colind, p.vals, x))
+    B.cg.set_option("tpr", 8)
+    B.cg.set_option("spmv", 0)
+
+
+def _random_csr(n, seed, max_len, empty_every=0, unsorted=False):
+    """Irregular CSR with ragged rows, optional empty rows, unsorted / duplicate columns."""
+    u = gi.hash_uniform(seed, 2, np.arange(n, dtype=np.uint64))
+    lens = (u * (max_len + 1)).astype(np.int64)
+    if empty_every:
+        lens[::empty_every] = 0
+    rp = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(lens, out=rp[1:])
+    nnz = int(rp[-1])
+    ci = (gi.hash_uniform(seed + 1, 2, np.arange(nnz, dtype=np.uint64)) * n).astype(np.int32)
+    va = 2 * gi.hash_uniform(seed + 2, 2, np.arange(nnz, dtype=np.uint64)) - 1
+    if not unsorted:
+        for i in range(n):
+            ci[rp[i]:rp[i + 1]].sort()
+    return rp.astype(np.int32), ci, va
+
+
+@pytest.mark.parametrize("n,max_len,empty_every", [(1, 1, 0), (2, 3, 0), (31, 5, 3), (33, 40, 0),
+                                                   (1000, 31, 7), (4097, 70, 5), (5000, 300, 11)])
+def test_spmv_irregular_matrices(cgmod, orc, n, max_len, empty_every):
+    """Ragged tails, empty rows, duplicate and unsorted columns, rows longer than a tile
+    (the streamed variant must refuse those and fall back), nnz not a multiple of 4."""
+    rp, ci, va = _random_csr(n, 1000 + n, max_len, empty_every, unsorted=True)
+    cg = cgmod.CG(dev(rp), dev(ci), dev(va))
+    x = gi.seeded_vector(5, n)
+    want = orc.spmv(rp, ci, va, x)
+    denom = orc.absrow(rp, ci, va, x) + 1e-300
+    for variant in (1, 2):
+        cg.set_option("spmv", variant)
+        if variant == 2 and not cg.info("stream_ok"):
+            assert cg.info("spmv") == 1
+        y = cg.spmv(dev(x)).cpu().numpy()
+        assert np.all(np.abs(y - want) <= SPMV_TOL * denom), (n, variant)
+    assert cg.check_csr()
+    cg.close()
+
+
+@pytest.mark.parametrize("n", [1, 2, 255, 256, 257, 132651, 1 << 20])
+def test_dot_parity(bound, orc, n):
+    B = bound(0)
+    a, b = gi.seeded_vector(61, n), gi.seeded_vector(62, n)
+    cg = B.cg if n == B.p.n else None
+    if cg is None:
+        rp = np.arange(n + 1, dtype=np.int32)
+        cgm = __import__("paper_1107_0538_b200")
+        cg = cgm.CG(dev(rp), dev(np.arange(n, dtype=np.int32)), dev(np.ones(n)))
+    got = cg.dot(dev(a), dev(b))
+    ref = orc.dot_ld(a, b)
+    assert abs(got - ref) <= 1e-15 * np.sum(np.abs(a * b)) * max(1.0, math.log2(n))
+    assert got == cg.dot(dev(a), dev(b))                     # bitwise reproducible
+    if cg is not B.cg:
+        cg.close()
+
+
+# ---------------------------------------------------------------- cg_solve
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_solve_parity_persistent(bound, orc, cfg, variant):
+    B = bound(cfg)
+    p = B.p
+    B.cg.set_option("loop", 0)
+    B.cg.set_option("spmv", variant)
+    ref = oracle_solve(orc, p, ("cg", cfg))
+    x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+    check_solve_parity(res, x, ref)
+    assert res.status == 0
+    # the recurrence residual the GPU reports is the true residual of the x it returns
+    true_r = p.b - orc.spmv_ld(p.rowptr, p.colind, p.vals, x.cpu().numpy())
+    assert np.linalg.norm(true_r) / np.linalg.norm(p.b) <= 2 * p.rtol
+    assert abs(res.resnorm - res.hist[-1].item()) == 0.0
+    if p.xstar is not None:
+        assert np.linalg.norm(x.cpu().numpy() - p.xstar) / np.linalg.norm(p.xstar) < 1e-7
+    B.cg.set_option("spmv", 0)
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_loop_modes_agree_bitwise(bound, cfg):
+    """Persistent kernel, CUDA-graph replay and plain launches share the phase code and the
+    reduction order: identical bits.  Also run-to-run reproducibility (a cheap race detector)."""
+    B = bound(cfg)
+    p = B.p
+    outs = []
+    for variant in (1, 2):
+        B.cg.set_option("spmv", variant)
+        per_mode = []
+        for loop in (0, 1, 2, 0):
+            B.cg.set_option("loop", loop)
+            x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+            per_mode.append((x.cpu().numpy().copy(), res.hist.cpu().numpy().copy(), res.iters, res.status))
+        for other in per_mode[1:]:
+            assert other[2] == per_mode[0][2] and other[3] == per_mode[0][3]
+            assert np.array_equal(other[1], per_mode[0][1])
+            assert np.array_equal(other[0], per_mode[0][0])
+        outs.append(per_mode[0])
+    B.cg.set_option("loop", 0)
+    B.cg.set_option("spmv", 0)
+    assert abs(outs[0][2] - outs[1][2]) <= 1           # the two SpMV variants differ only by rounding
+
+
+def test_graph_chunk_sizes_and_launch_count(bound):
+    B = bound(0)
+    p = B.p
+    B.cg.set_option("loop", 0)
+    x0, r0 = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+    assert B.cg.info("launches") == 1
+    for chunk in (2, 8, 64):
+        B.cg.set_option("loop", 1)
+        B.cg.set_option("chunk", chunk)
+        x, r = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+        assert r.iters == r0.iters and torch.equal(x, x0)
+        assert B.cg.info("launches") == 3 + 3 * chunk * math.ceil(r.iters / chunk)
+    B.cg.set_option("chunk", 32)
+    B.cg.set_option("loop", 0)
+
+
+def test_handworked_2x2(cgmod):
+    """tests/golden/cg_2x2_handworked.txt through the CUDA path."""
+    cg = cgmod.CG(dev(np.array([0, 2, 4], dtype=np.int32)), dev(np.array([0, 1, 0, 1], dtype=np.int32)),
+                  dev(np.array([2.0, -1.0, -1.0, 2.0])))
+    for loop in (0, 1, 2):
+        cg.set_option("loop", loop)
+        x, res = cg.solve(dev(np.array([1.0, 0.0])), rtol=1e-14, maxit=10)
+        assert res.iters == 2 and res.status == 0
+        np.testing.assert_allclose(res.hist.cpu().numpy(), [1.0, 0.5, 0.0], atol=1e-16)
+        np.testing.assert_allclose(x.cpu().numpy(), [2 / 3, 1 / 3], rtol=1e-15)
+    cg.close()
+
+
+def test_conventions_and_edge_cases(bound, cgmod, orc):
+    B = bound(0)
+    p = B.p
+    for loop in (0, 1, 2):
+        B.cg.set_option("loop", loop)
+        # b = 0 -> x = 0, k = 0, converged, hist = [0]
+        x, res = B.cg.solve(torch.zeros_like(B.b), x0=torch.ones_like(B.b), rtol=1e-10, maxit=10)
+        assert res.iters == 0 and res.status == 0 and float(x.abs().max()) == 0.0
+        assert res.hist.cpu().tolist() == [0.0]
+        # rtol = 0 -> exactly maxit iterations, status 1
+        x, res = B.cg.solve(B.b, rtol=0.0, maxit=7)
+        ref = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=0.0, maxit=7)
+        assert res.iters == 7 and res.status == 1
+        assert np.linalg.norm(x.cpu().numpy() - ref.x) / np.linalg.norm(ref.x) < 1e-12
+        # maxit = 0 -> no iteration, x = x0
+        x, res = B.cg.solve(B.b, rtol=1e-10, maxit=0)
+        assert res.iters == 0 and res.status == 1 and float(x.abs().max()) == 0.0
+        assert abs(res.resnorm - np.linalg.norm(p.b)) <= 1e-13 * np.linalg.norm(p.b)
+        # x0 = solution -> zero iterations, converged
+        ref = oracle_solve(orc, p, ("cg", 0))
+        x, res = B.cg.solve(B.b, x0=dev(ref.x), rtol=1e-9, maxit=10)
+        assert res.iters == 0 and res.status == 0
+        # nonzero x0 is used as the starting point (r0 = b - A x0)
+        x0 = gi.seeded_vector(77, p.n)
+        x, res = B.cg.solve(B.b, x0=dev(x0), rtol=p.rtol, maxit=p.maxit)
+        ref2 = orc.cg(p.rowptr, p.colind, p.vals, p.b, x0=x0, rtol=p.rtol, maxit=p.maxit)
+        check_solve_parity(res, x, ref2)
+    B.cg.set_option("loop", 0)
+    # breakdown: -A is negative definite
+    neg = cgmod.CG(dev(p.rowptr), dev(p.colind), dev(-p.vals))
+    for loop in (0, 1, 2):
+        neg.set_option("loop", loop)
+        x, res = neg.solve(B.b, rtol=1e-10, maxit=10)
+        assert res.status == 2 and res.iters == 0
+        assert float(x.abs().max()) == 0.0
+    neg.close()
+
+
+def test_invalid_arguments(bound, cgmod):
+    B = bound(0)
+    L = cgmod.lib()
+    n = B.p.n
+    x = torch.zeros(n + 1, dtype=torch.float64, device="cuda")
+    h, b = B.cg.h, B.b.data_ptr()
+    assert L.cg_solve(h, b, x.data_ptr(), float("nan"), 10, None, None, None, None) == -1
+    assert L.cg_solve(h, b, x.data_ptr(), -1.0, 10, None, None, None, None) == -1
+    assert L.cg_solve(h, b, x.data_ptr(), 1e-3, -1, None, None, None, None) == -1
+    assert L.cg_solve(h, b, None, 1e-3, 10, None, None, None, None) == -1
+    assert L.cg_solve(h, b, x[1:].data_ptr(), 1e-3, 10, None, None, None, None) == -1   # misaligned
+    assert L.cg_spmv(h, b, b, None) == -1                                                # aliasing
+    with pytest.raises(cgmod.CGError):
+        cgmod.cg_create(n, B.p.nnz, B.cg.rowptr.data_ptr(), B.cg.colind.data_ptr(),
+                        B.cg.vals.data_ptr(), B.cg.workspace.data_ptr(), 1024)            # workspace too small
+    with pytest.raises(cgmod.CGError):
+        cgmod.cg_create(0, 0, B.cg.rowptr.data_ptr(), B.cg.colind.data_ptr(), B.cg.vals.data_ptr(),
+                        B.cg.workspace.data_ptr(), B.cg.workspace.numel())
+    with pytest.raises(cgmod.CGError):
+        B.cg.set_option("nonsense", 1)
+    # a broken CSR structure is reported by cg_check_csr
+    bad_ci = B.cg.colind.clone()
+    bad_ci[5] = n + 3
+    bad = cgmod.CG(B.cg.rowptr, bad_ci, B.cg.vals)
+    assert not bad.check_csr()
+    bad.close()
+    assert B.cg.check_csr()
+
+
+def test_solve_host_end_to_end(bound, orc):
+    B = bound(2)
+    p = B.p
+    hb = torch.from_numpy(p.b).pin_memory()
+    hx = torch.zeros(p.n, dtype=torch.float64).pin_memory()
+    hh = torch.zeros(p.maxit + 1, dtype=torch.float64).pin_memory()
+    st, it, res = B.cg.solve_host(hb, hx, p.rtol, p.maxit, hh)
+    ref = oracle_solve(orc, p, ("cg", 2))
+    assert st == 0 and abs(it - ref.iters) <= max(1, int(0.02 * ref.iters))
+    assert np.linalg.norm(hx.numpy() - ref.x) / np.linalg.norm(ref.x) <= X_TOL
+    k = min(50, it)
+    assert np.max(np.abs(hh.numpy()[:k + 1] - ref.hist[:k + 1]) / ref.hist[:k + 1]) <= HIST_TOL
+    assert hh.numpy()[it] == res
+
+
+# ---------------------------------------------------------------- Jacobi PCG (8(f) rank 1)
+
+@pytest.mark.parametrize("cfg,grid", [(0, None), (4, 32)])
+def test_jacobi_parity(bound, orc, cfg, grid):
+    B = bound(cfg, grid)
+    p = B.p
+    diag = np.array([p.vals[p.rowptr[i]:p.rowptr[i + 1]][p.colind[p.rowptr[i]:p.rowptr[i + 1]] == i].sum()
+                     for i in range(p.n)])
+    ref = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit, dinv=1.0 / diag)
+    for loop in (0, 1):
+        B.cg.set_option("loop", loop)
+        x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit, jacobi=True)
+        check_solve_parity(res, x, ref)
+    B.cg.set_option("loop", 0)
+    if cfg == 4:
+        plain = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+        assert ref.iters < plain.iters / 3          # the point of the preconditioner on contrast
+
+
+# ---------------------------------------------------------------- full-size config 4
+
+@pytest.fixture(scope="module")
+def config4(cgmod, problems):
+    B = Bound(cgmod, problems(4))
+    yield B
+    B.cg.close()
+
+
+def test_config4_spmv_full_size(config4, orc):
+    """160^3, NNZ = 109 215 352, in the launch configuration bench.py times."""
+    B = config4
+    p = B.p
+    assert p.n == 4096000 and p.nnz == 109215352
+    x = gi.seeded_vector(104, p.n)
+    want = orc.spmv(p.rowptr, p.colind, p.vals, x)
+    denom = orc.absrow(p.rowptr, p.colind, p.vals, x)
+    for variant in (1, 2):
+        B.cg.set_option("spmv", variant)
+        y = B.cg.spmv(dev(x)).cpu().numpy()
+        assert (np.abs(y - want) / denom).max() <= SPMV_TOL
+    B.cg.set_option("spmv", 0)
+    ones = torch.ones(p.n, dtype=torch.float64, device="cuda")
+    y1 = B.cg.spmv(ones).cpu().numpy()
+    assert np.all(np.abs(y1 - 0.01) <= SPMV_TOL * orc.absrow(p.rowptr, p.colind, p.vals, np.ones(p.n)))
+
+
+def test_config4_fixed_iterations(config4, orc):
+    """Reading 14: on the ill-conditioned config a fixed-iteration run (rtol = 0, maxit = 50)
+    must match the oracle's history (first 50) and x to 1e-8."""
+    B = config4
+    p = B.p
+    ref = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=0.0, maxit=50)
+    x, res = B.cg.solve(B.b, rtol=0.0, maxit=50)
+    check_solve_parity(res, x, ref)
+    assert res.iters == 50 and res.status == 1
