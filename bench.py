@@ -159,6 +159,10 @@ def main():
     ap.add_argument("--loop", type=int, default=0)
     ap.add_argument("--spmv", type=int, default=0)
     ap.add_argument("--fixed-iters-160", type=int, default=200)
+    ap.add_argument("--profile", type=int, default=None, metavar="CFG",
+                    help="profiling aid (ncu): only run 3 fixed-work solves of config CFG and exit")
+    ap.add_argument("--profile-iters", type=int, default=6)
+    ap.add_argument("--ctas-per-sm", type=int, default=0)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -208,11 +212,38 @@ def main():
         rp, ci, va = (torch.from_numpy(a).to(dev) for a in (p.rowptr, p.colind, p.vals))
         return cg.CG(rp, ci, va)
 
+    if args.profile is not None:
+        pp = cg_inputs.make_config(args.profile)
+        Ap = bind(pp)
+        Ap.set_option("loop", args.loop)
+        Ap.set_option("spmv", args.spmv)
+        if args.ctas_per_sm:
+            Ap.set_option("ctas_per_sm", args.ctas_per_sm)
+        bp = torch.from_numpy(pp.b).to(dev)
+        xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
+        out = []
+        for rep in range(3):
+            xp.zero_()
+            flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            st, it, res = cg.cg_solve(Ap.h, bp.data_ptr(), xp.data_ptr(), 0.0, args.profile_iters, None,
+                                      torch.cuda.current_stream().cuda_stream)
+            e1.record()
+            torch.cuda.synchronize()
+            out.append(e0.elapsed_time(e1) * 1e3 / max(it, 1))
+        print(json.dumps({"profile_config": args.profile, "iters": args.profile_iters, "us_per_iteration": out,
+                          "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid")}))
+        Ap.close()
+        return
+
     # ------------------------------------------------------------ the metric's workload (config 2)
     p = cg_inputs.make_config(WORKLOAD_CFG)
     A = bind(p)
     A.set_option("loop", args.loop)
     A.set_option("spmv", args.spmv)
+    if args.ctas_per_sm:
+        A.set_option("ctas_per_sm", args.ctas_per_sm)
     b = torch.from_numpy(p.b).to(dev)
     x = torch.zeros(p.n, dtype=torch.float64, device=dev)
     hist = torch.zeros(p.maxit + 1, dtype=torch.float64, device=dev)
@@ -322,6 +353,8 @@ def main():
             A4 = bind(p4)
             A4.set_option("loop", args.loop)
             A4.set_option("spmv", args.spmv)
+            if args.ctas_per_sm:
+                A4.set_option("ctas_per_sm", args.ctas_per_sm)
             b4 = torch.from_numpy(p4.b).to(dev)
             x4 = torch.zeros(p4.n, dtype=torch.float64, device=dev)
             K = args.fixed_iters_160

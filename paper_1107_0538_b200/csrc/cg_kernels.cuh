@@ -326,9 +326,32 @@ __device__ __forceinline__ double phase_spmv_stream(const Params& P, const doubl
         mbar_wait(&sm->full[warp][sidx], (phase_bits >> sidx) & 1u);
         phase_bits ^= (1u << sidx);
         __syncwarp();
-        double acc = 0.0;
-        for (int k = s - base; k < e - base; ++k)
-            acc = fma(st->vals[k], x[st->cols[k]], acc);
+        // kUnroll entries per trip: all shared-memory reads first, then all x gathers, then
+        // the FMAs into 3 independent accumulators (27 = 3 x 9 for the stencil rows).
+        constexpr int kUnroll = 9;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+        const int ks = s - base, ke = e - base;
+        for (int k = ks; k < ke; k += kUnroll) {
+            double v[kUnroll];
+            int c[kUnroll];
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u) {
+                const bool ok = k + u < ke;
+                const int kk = ok ? k + u : ke - 1;          // stay inside this row's span
+                c[u] = st->cols[kk];
+                v[u] = ok ? st->vals[kk] : 0.0;
+            }
+            double xv[kUnroll];
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u) xv[u] = x[c[u]];
+#pragma unroll
+            for (int u = 0; u < kUnroll; u += 3) {
+                a0 = fma(v[u], xv[u], a0);
+                a1 = fma(v[u + 1], xv[u + 1], a1);
+                a2 = fma(v[u + 2], xv[u + 2], a2);
+            }
+        }
+        const double acc = (a0 + a1) + a2;
         if (row < P.n) {
             y[row] = acc;
             if (DOT) dot = fma(acc, x[row], dot);
@@ -372,6 +395,19 @@ __device__ __forceinline__ void phase_init_residual(const Params& P, int cta, in
     if (P.precond) { t = block_sum(arz, sm); if (threadIdx.x == 0) P.part3[cta] = t; }
 }
 
+// Streaming accesses for x: touched exactly once per iteration (read + write in K2), so it
+// is marked evict-first and leaves the L2 to p, q, r, which are re-read by the next phase.
+__device__ __forceinline__ double2 ld_cs_f64x2(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_cs_f64x2(double2* p, double2 v) {
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" :: "l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+
+constexpr int kVecUnroll = 4;     // double2 elements in flight per thread and array
+
 // K2: x += alpha p ; r -= alpha q ; partial r.r (and r.z with Jacobi).
 __device__ __forceinline__ void phase_update_xr(const Params& P, double alpha, int cta, int G,
                                                 double* sm) {
@@ -379,22 +415,34 @@ __device__ __forceinline__ void phase_update_xr(const Params& P, double alpha, i
     double arr = 0.0, arz = 0.0;
     const long long np2 = P.n >> 1;
     const long long stride = (long long)G * kThreads;
-    double2* __restrict__ x2 = reinterpret_cast<double2*>(P.x);
-    double2* __restrict__ r2 = reinterpret_cast<double2*>(P.r);
-    const double2* __restrict__ p2 = reinterpret_cast<const double2*>(P.p);
-    const double2* __restrict__ q2 = reinterpret_cast<const double2*>(P.q);
-    const double2* __restrict__ d2 = reinterpret_cast<const double2*>(P.dinv);
-#pragma unroll 2
-    for (long long i = (long long)cta * kThreads + threadIdx.x; i < np2; i += stride) {
-        double2 xv = x2[i], rv = r2[i];
-        const double2 pv = p2[i], qv = q2[i];
-        xv.x = fma(alpha, pv.x, xv.x); xv.y = fma(alpha, pv.y, xv.y);
-        rv.x = fma(na, qv.x, rv.x);    rv.y = fma(na, qv.y, rv.y);
-        x2[i] = xv; r2[i] = rv;
-        arr = fma(rv.x, rv.x, arr); arr = fma(rv.y, rv.y, arr);
-        if (P.precond) {
-            const double2 dv = d2[i];
-            arz = fma(rv.x, dv.x * rv.x, arz); arz = fma(rv.y, dv.y * rv.y, arz);
+    double2* x2 = reinterpret_cast<double2*>(P.x);
+    double2* r2 = reinterpret_cast<double2*>(P.r);
+    const double2* p2 = reinterpret_cast<const double2*>(P.p);
+    const double2* q2 = reinterpret_cast<const double2*>(P.q);
+    const double2* d2 = reinterpret_cast<const double2*>(P.dinv);
+    for (long long i0 = (long long)cta * kThreads + threadIdx.x; i0 < np2; i0 += stride * kVecUnroll) {
+        double2 xv[kVecUnroll], rv[kVecUnroll], pv[kVecUnroll], qv[kVecUnroll], dv[kVecUnroll];
+#pragma unroll
+        for (int u = 0; u < kVecUnroll; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < np2) {
+                xv[u] = ld_cs_f64x2(x2 + i); rv[u] = r2[i]; pv[u] = p2[i]; qv[u] = q2[i];
+                if (P.precond) dv[u] = d2[i];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kVecUnroll; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < np2) {
+                xv[u].x = fma(alpha, pv[u].x, xv[u].x); xv[u].y = fma(alpha, pv[u].y, xv[u].y);
+                rv[u].x = fma(na, qv[u].x, rv[u].x);    rv[u].y = fma(na, qv[u].y, rv[u].y);
+                st_cs_f64x2(x2 + i, xv[u]); r2[i] = rv[u];
+                arr = fma(rv[u].x, rv[u].x, arr); arr = fma(rv[u].y, rv[u].y, arr);
+                if (P.precond) {
+                    arz = fma(rv[u].x, dv[u].x * rv[u].x, arz);
+                    arz = fma(rv[u].y, dv[u].y * rv[u].y, arz);
+                }
+            }
         }
     }
     if ((P.n & 1) && cta == G - 1 && threadIdx.x == kThreads - 1) {      // odd tail element
@@ -413,16 +461,26 @@ __device__ __forceinline__ void phase_update_xr(const Params& P, double alpha, i
 __device__ __forceinline__ void phase_update_p(const Params& P, double beta, int cta, int G) {
     const long long np2 = P.n >> 1;
     const long long stride = (long long)G * kThreads;
-    double2* __restrict__ p2 = reinterpret_cast<double2*>(P.p);
-    const double2* __restrict__ r2 = reinterpret_cast<const double2*>(P.r);
-    const double2* __restrict__ d2 = reinterpret_cast<const double2*>(P.dinv);
-#pragma unroll 2
-    for (long long i = (long long)cta * kThreads + threadIdx.x; i < np2; i += stride) {
-        double2 pv = p2[i];
-        double2 rv = r2[i];
-        if (P.precond) { const double2 dv = d2[i]; rv.x *= dv.x; rv.y *= dv.y; }
-        pv.x = fma(beta, pv.x, rv.x); pv.y = fma(beta, pv.y, rv.y);
-        p2[i] = pv;
+    double2* p2 = reinterpret_cast<double2*>(P.p);
+    const double2* r2 = reinterpret_cast<const double2*>(P.r);
+    const double2* d2 = reinterpret_cast<const double2*>(P.dinv);
+    constexpr int U = 2 * kVecUnroll;
+    for (long long i0 = (long long)cta * kThreads + threadIdx.x; i0 < np2; i0 += stride * U) {
+        double2 pv[U], rv[U], dv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < np2) { pv[u] = p2[i]; rv[u] = r2[i]; if (P.precond) dv[u] = d2[i]; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < np2) {
+                if (P.precond) { rv[u].x *= dv[u].x; rv[u].y *= dv[u].y; }
+                pv[u].x = fma(beta, pv[u].x, rv[u].x); pv[u].y = fma(beta, pv[u].y, rv[u].y);
+                p2[i] = pv[u];
+            }
+        }
     }
     if ((P.n & 1) && cta == G - 1 && threadIdx.x == kThreads - 1) {
         const long long i = P.n - 1;
