@@ -217,6 +217,8 @@ def main():
         Ap = bind(pp)
         Ap.set_option("loop", args.loop)
         Ap.set_option("spmv", args.spmv)
+        if args.profile_iters % 2 == 0:
+            Ap.set_option("chunk", args.profile_iters)      # no no-op launches after the stop flag
         if args.ctas_per_sm:
             Ap.set_option("ctas_per_sm", args.ctas_per_sm)
         bp = torch.from_numpy(pp.b).to(dev)

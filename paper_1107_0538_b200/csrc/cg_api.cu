@@ -67,7 +67,7 @@ __global__ void k_diag_inv(Params P) {
 }
 
 template <int V>
-__global__ void __launch_bounds__(kThreads) k_spmv(Params P, const double* x, double* y) {
+__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_spmv(Params P, const double* x, double* y) {
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     stream_smem_init<V>(dyn_smem);
     uint32_t bits = 0;
@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(kThreads) k_dot_final(const double* part, int 
 // ---- Params from device memory so that a captured graph survives across solves.
 
 template <int V>
-__global__ void __launch_bounds__(kThreads) k_init_spmv(const Params* __restrict__ dp) {
+__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_init_spmv(const Params* __restrict__ dp) {
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     const Params P = *dp;
     stream_smem_init<V>(dyn_smem);
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(kThreads) k_init_spmv(const Params* __restrict
     phase_spmv<V, false>(P, P.x, P.q, blockIdx.x, gridDim.x, dyn_smem, bits);
 }
 
-__global__ void __launch_bounds__(kThreads) k_init_residual(const Params* __restrict__ dp) {
+__global__ void __launch_bounds__(kThreads, 2) k_init_residual(const Params* __restrict__ dp) {
     __shared__ double sm[kWarps + 1];
     const Params P = *dp;
     phase_init_residual(P, blockIdx.x, gridDim.x, sm);
@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(kThreads) k_init_scalars(const Params* __restr
 }
 
 template <int V>
-__global__ void __launch_bounds__(kThreads) k1_spmv_dot(const Params* __restrict__ dp, int s) {
+__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k1_spmv_dot(const Params* __restrict__ dp, int s) {
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     __shared__ double sm[kWarps + 1];
     const Params P = *dp;
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(kThreads) k1_spmv_dot(const Params* __restrict
     if (threadIdx.x == 0) P.part0[blockIdx.x] = t;
 }
 
-__global__ void __launch_bounds__(kThreads) k2_update_xr(const Params* __restrict__ dp, int s) {
+__global__ void __launch_bounds__(kThreads, 2) k2_update_xr(const Params* __restrict__ dp, int s) {
     __shared__ double sm[kWarps + 1];
     const Params P = *dp;
     if (P.scal->st[s].stop) return;
@@ -164,10 +164,10 @@ __global__ void __launch_bounds__(kThreads) k2_update_xr(const Params* __restric
         return;
     }
     const double alpha = P.scal->st[s].rz / pq;
-    phase_update_xr(P, alpha, blockIdx.x, gridDim.x, sm);
+    phase_update_xr<4>(P, alpha, blockIdx.x, gridDim.x, sm);
 }
 
-__global__ void __launch_bounds__(kThreads) k3_update_p(const Params* __restrict__ dp, int s) {
+__global__ void __launch_bounds__(kThreads, 2) k3_update_p(const Params* __restrict__ dp, int s) {
     __shared__ double sm[kWarps + 1];
     const Params P = *dp;
     Scal* S = P.scal;
@@ -196,14 +196,14 @@ __global__ void __launch_bounds__(kThreads) k3_update_p(const Params* __restrict
         if (P.hist) P.hist[k] = res;
         if (stop) { S->out_iters = k; S->out_status = status; S->out_res = res; }
     }
-    if (!stop) phase_update_p(P, beta, blockIdx.x, gridDim.x);
+    if (!stop) phase_update_p<4>(P, beta, blockIdx.x, gridDim.x);
 }
 
 // ---- loop mode 0: the whole solve as ONE cooperative persistent kernel.
 // Scalars live in registers, identical in every CTA; three grid barriers per
 // iteration (after K1, K2, K3); nothing leaves the device until the end.
 template <int V>
-__global__ void __launch_bounds__(kThreads) k_persistent(Params P) {
+__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_persistent(Params P) {
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     __shared__ double sm[kWarps + 1];
     const int cta = blockIdx.x, G = gridDim.x;
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(kThreads) k_persistent(Params P) {
         if (!(pq > 0.0) || !is_finite(pq)) { stop = 1; status = CG_BREAKDOWN; break; }
         const double alpha = rz / pq;
         // K2
-        phase_update_xr(P, alpha, cta, G, sm);
+        phase_update_xr<(V == 2 ? 4 : 2)>(P, alpha, cta, G, sm);
         grid_barrier(&S->bar, G, epoch);
         // scalar beta, continue-condition
         const double rr_new = sum_partials(P.part1, G, sm);
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(kThreads) k_persistent(Params P) {
         if (res <= thresh) { stop = 1; status = CG_OK; break; }
         if (k >= P.maxit) { stop = 1; status = CG_MAXIT; break; }
         // K3
-        phase_update_p(P, beta, cta, G);
+        phase_update_p<(V == 2 ? 4 : 2)>(P, beta, cta, G);
         grid_barrier(&S->bar, G, epoch);
     }
     if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(rr); }
@@ -323,7 +323,7 @@ template <int V> static int setup_variant(cg_handle* h) {
     int bps = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_persistent<V>, kThreads, smem));
     if (bps < 1) { snprintf(g_cuda_err, sizeof(g_cuda_err), "persistent kernel does not fit an SM"); return CG_ECUDA; }
-    int want = h->ctas_per_sm > 0 ? h->ctas_per_sm : (V == 2 ? 1 : 4);
+    int want = h->ctas_per_sm > 0 ? h->ctas_per_sm : (V == 2 ? 1 : 2);
     if (want > bps) want = bps;
     int g = h->sms * want;
     if (g > kMaxGrid) g = kMaxGrid;

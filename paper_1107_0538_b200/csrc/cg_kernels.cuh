@@ -22,7 +22,10 @@ namespace cgk {
 
 constexpr int kThreads = 256;       // threads per CTA, every kernel
 constexpr int kWarps = kThreads / 32;
-constexpr int kMaxGrid = 2048;      // capacity of each partials array
+constexpr int kMaxGrid = 2048;
+// ptxas schedules for ILP only when told the occupancy target: 1 CTA/SM for the streamed
+// variant (shared-memory bound anyway), 2 for the sub-warp variant.
+template <int V> struct MinBlocks { static constexpr int value = (V == 2) ? 1 : 2; };      // capacity of each partials array
 
 // SpMV variant B (bulk-async streamed tiles): each warp owns a private ring of
 // kStages tiles of kTileRows rows; a tile's nnz span must fit kTileCap entries.
@@ -89,6 +92,11 @@ __device__ __forceinline__ double ld_stream_f64(const double* p) {
 __device__ __forceinline__ int ld_stream_s32(const int* p) {
     int v;
     asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ld_global_f64(const double* p) {
+    double v;   // explicit global-space load (vectors are read AND written inside one launch: no .nc)
+    asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
@@ -178,7 +186,7 @@ __device__ __forceinline__ double phase_spmv_vector(const Params& P, const doubl
                 const double v1 = b1 ? ld_stream_f64(vals + k1) : 0.0;
                 const double v2 = b2 ? ld_stream_f64(vals + k2) : 0.0;
                 const double v3 = b3 ? ld_stream_f64(vals + k3) : 0.0;
-                const double x0 = x[c0], x1 = x[c1], x2 = x[c2], x3 = x[c3];
+                const double x0 = ld_global_f64(x + c0), x1 = ld_global_f64(x + c1), x2 = ld_global_f64(x + c2), x3 = ld_global_f64(x + c3);
                 acc = fma(v0, x0, acc);
                 acc = fma(v1, x1, acc);
                 acc = fma(v2, x2, acc);
@@ -343,7 +351,7 @@ __device__ __forceinline__ double phase_spmv_stream(const Params& P, const doubl
             }
             double xv[kUnroll];
 #pragma unroll
-            for (int u = 0; u < kUnroll; ++u) xv[u] = x[c[u]];
+            for (int u = 0; u < kUnroll; ++u) xv[u] = ld_global_f64(x + c[u]);
 #pragma unroll
             for (int u = 0; u < kUnroll; u += 3) {
                 a0 = fma(v[u], xv[u], a0);
@@ -406,9 +414,11 @@ __device__ __forceinline__ void st_cs_f64x2(double2* p, double2 v) {
     asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" :: "l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
 
-constexpr int kVecUnroll = 4;     // double2 elements in flight per thread and array
+// VU = double2 elements in flight per thread and array.  It only batches the loads; the
+// per-thread accumulation order (hence every bit of the result) does not depend on it.
 
 // K2: x += alpha p ; r -= alpha q ; partial r.r (and r.z with Jacobi).
+template <int kVecUnroll>
 __device__ __forceinline__ void phase_update_xr(const Params& P, double alpha, int cta, int G,
                                                 double* sm) {
     const double na = -alpha;
@@ -458,6 +468,7 @@ __device__ __forceinline__ void phase_update_xr(const Params& P, double alpha, i
 }
 
 // K3: p = r + beta p   (Jacobi: p = D^-1 r + beta p).
+template <int kVecUnroll>
 __device__ __forceinline__ void phase_update_p(const Params& P, double beta, int cta, int G) {
     const long long np2 = P.n >> 1;
     const long long stride = (long long)G * kThreads;
