@@ -163,6 +163,10 @@ def main():
                     help="profiling aid (ncu): only run 3 fixed-work solves of config CFG and exit")
     ap.add_argument("--profile-iters", type=int, default=6)
     ap.add_argument("--ctas-per-sm", type=int, default=0)
+    ap.add_argument("--lookahead", type=int, default=None)
+    ap.add_argument("--resident", type=int, default=None)
+    ap.add_argument("--trace", action="store_true",
+                    help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -221,9 +225,14 @@ def main():
             Ap.set_option("chunk", args.profile_iters)      # no no-op launches after the stop flag
         if args.ctas_per_sm:
             Ap.set_option("ctas_per_sm", args.ctas_per_sm)
+        if args.lookahead is not None:
+            Ap.set_option("lookahead", args.lookahead)
+        if args.resident is not None:
+            Ap.set_option("resident", args.resident)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []
+        tr = Ap.trace(args.profile_iters) if (args.trace and args.loop == 0) else None
         for rep in range(3):
             xp.zero_()
             flush_l2()
@@ -234,8 +243,25 @@ def main():
             e1.record()
             torch.cuda.synchronize()
             out.append(e0.elapsed_time(e1) * 1e3 / max(it, 1))
-        print(json.dumps({"profile_config": args.profile, "iters": args.profile_iters, "us_per_iteration": out,
-                          "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid")}))
+        rec = {"profile_config": args.profile, "iters": args.profile_iters, "us_per_iteration": out,
+               "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid")}
+        if tr is not None:
+            # [cta, iter, slot] clock64 stamps -> cycles per interval; skip the first 2 iterations
+            full = tr.cpu().numpy().astype(np.int64)
+            st = full[:, args.profile_iters, :]
+            rec["ring_stats"] = {"producer_wait_cycles": float(st[:, 0].mean()), "producer_total_cycles": float(st[:, 1].mean()),
+                                 "tiles_issued": float(st[:, 2].mean()), "consumer_warp0_full_wait_cycles": float(st[:, 3].mean())}
+            t = full[:, 2:args.profile_iters - 1, :]
+            names = ["K1 work", "barrier 1", "alpha + K2 work", "barrier 2", "beta", "K3 work", "barrier 3"]
+            d = np.diff(t[:, :, :8], axis=2)
+            if t.shape[2] >= 16 and t[:, :, 8:].any():
+                dd = np.diff(t[:, :, 8:], axis=2)
+                rec["barrier3_detail_cycles"] = {nm: float(dd[:, :, i].mean()) for i, nm in enumerate(
+                    ["cta reduce", "publish", "poll", "syncwarp", "fence", "totals", "final sync"])}
+            rec["trace_cycles"] = {nm: {"mean": float(d[:, :, i].mean()), "max_cta": float(d[:, :, i].max(axis=0).mean()),
+                                        "min_cta": float(d[:, :, i].min(axis=0).mean())} for i, nm in enumerate(names)}
+            rec["trace_cycles"]["iteration"] = float((t[:, :, 7] - t[:, :, 0]).mean())
+        print(json.dumps(rec))
         Ap.close()
         return
 

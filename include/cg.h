@@ -127,6 +127,14 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
 int cg_set_option(cg_handle* h, const char* name, int64_t value);
 int cg_get_info(cg_handle* h, const char* name, int64_t* value);
 
+/* Phase trace of the persistent loop (loop mode 0), a profiling aid: with a non-NULL
+ * d_trace (device uint64[grid * (iters + 1) * 16], grid = cg_get_info "grid"), thread 0 of every
+ * CTA stores clock64() at 8 points (slots 0-7; slots 8-15 detail the third grid barrier) of each of the first `iters` iterations of later
+ * solves: [0] iteration start, [1] K1 done, [2] past barrier 1, [3] K2 done, [4] past
+ * barrier 2, [5] beta known, [6] K3 done, [7] past barrier 3.  Layout [cta][iter][slot].
+ * NULL or iters = 0 switches it off (the default).  The buffer is borrowed. */
+int cg_set_trace(cg_handle* h, uint64_t* d_trace, int64_t iters);
+
 /* Frees the host struct (and any CUDA graph).  Device memory is the caller's. */
 int cg_destroy(cg_handle* h);
 

@@ -33,6 +33,7 @@ SIGNATURES = {
                                        ctypes.POINTER(_f64), _vp]),
     "cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, _f64, _i64, _vp, ctypes.POINTER(_i64),
                                      ctypes.POINTER(_f64), _vp, _sz, _vp]),
+    "cg_set_trace": (ctypes.c_int, [_vp, _vp, _i64]),
     "cg_set_option": (ctypes.c_int, [_vp, ctypes.c_char_p, _i64]),
     "cg_get_info": (ctypes.c_int, [_vp, ctypes.c_char_p, ctypes.POINTER(_i64)]),
     "cg_destroy": (ctypes.c_int, [_vp]),
@@ -147,6 +148,12 @@ def cg_set_option(h: int, name: str, value: int) -> None:
         raise CGError(rc, f"cg_set_option({name}={value})")
 
 
+def cg_set_trace(h: int, d_trace: Optional[int], iters: int) -> None:
+    rc = lib().cg_set_trace(h, d_trace, iters)
+    if rc != 0:
+        raise CGError(rc, "cg_set_trace")
+
+
 def cg_get_info(h: int, name: str) -> int:
     out = _i64()
     rc = lib().cg_get_info(h, name.encode(), ctypes.byref(out))
@@ -201,6 +208,18 @@ class CG:
 
     def info(self, name):
         return cg_get_info(self.h, name)
+
+    def trace(self, iters: int):
+        """Switch the persistent loop's phase trace on (returns the uint64 device tensor
+        [grid, iters + 1, 16] later solves fill (row `iters`: producer / wait statistics)) or, with iters = 0, off."""
+        if iters <= 0:
+            cg_set_trace(self.h, None, 0)
+            self._trace = None
+            return None
+        self._trace = self.torch.zeros((self.info("grid"), iters + 1, 16), dtype=self.torch.int64,
+                                       device=self.device)
+        cg_set_trace(self.h, self._trace.data_ptr(), iters)
+        return self._trace
 
     def check_csr(self) -> bool:
         return cg_check_csr(self.h, self._stream()) == 0

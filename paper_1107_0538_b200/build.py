@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SOURCES = [os.path.join(HERE, "csrc", "cg_api.cu")]
-DEPS = SOURCES + [os.path.join(HERE, "csrc", "cg_kernels.cuh"), os.path.join(ROOT, "include", "cg.h")]
+DEPS = SOURCES + [os.path.join(HERE, "csrc", "cg_kernels.cuh"), os.path.join(HERE, "csrc", "cg_stream.cuh"), os.path.join(HERE, "csrc", "cg_stream_kernels.cuh"), os.path.join(ROOT, "include", "cg.h")]
 LIB = os.path.join(HERE, "libcg_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]

@@ -2,6 +2,7 @@
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -shared -Xcompiler -fPIC
 #include "../../include/cg.h"
 #include "cg_kernels.cuh"
+#include "cg_stream_kernels.cuh"
 
 #include <math.h>
 #include <stdlib.h>
@@ -66,12 +67,16 @@ __global__ void k_diag_inv(Params P) {
     }
 }
 
-template <int V>
-__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_spmv(Params P, const double* x, double* y) {
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
-    stream_smem_init<V>(dyn_smem);
-    uint32_t bits = 0;
-    phase_spmv<V, false>(P, x, y, blockIdx.x, gridDim.x, dyn_smem, bits);
+// ---- generic variant (spmv = 1): sub-warp per row straight from global memory; any CSR matrix.
+__global__ void __launch_bounds__(kThreads, 2) k_spmv(Params P, const double* x, double* y) {
+    phase_spmv_vector_dispatch<false>(P, x, y, blockIdx.x, gridDim.x);
+}
+
+// padded copy of rowptr for the streamed variants' 36-int bulk copies
+__global__ void k_pad_rowptr(const int* __restrict__ rowptr, long long n, int* __restrict__ out, long long total) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride)
+        out[i] = rowptr[i < n ? i : n];
 }
 
 __global__ void __launch_bounds__(kThreads) k_dot_partial(const double* __restrict__ a,
@@ -95,13 +100,9 @@ __global__ void __launch_bounds__(kThreads) k_dot_final(const double* part, int 
 // ---- stand-alone kernels of loop modes 1 (graph) and 2 (stepwise).  They read
 // ---- Params from device memory so that a captured graph survives across solves.
 
-template <int V>
-__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_init_spmv(const Params* __restrict__ dp) {
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
+__global__ void __launch_bounds__(kThreads, 2) k_init_spmv(const Params* __restrict__ dp) {
     const Params P = *dp;
-    stream_smem_init<V>(dyn_smem);
-    uint32_t bits = 0;
-    phase_spmv<V, false>(P, P.x, P.q, blockIdx.x, gridDim.x, dyn_smem, bits);
+    phase_spmv_vector_dispatch<false>(P, P.x, P.q, blockIdx.x, gridDim.x);
 }
 
 __global__ void __launch_bounds__(kThreads, 2) k_init_residual(const Params* __restrict__ dp) {
@@ -140,16 +141,12 @@ __global__ void __launch_bounds__(kThreads) k_init_scalars(const Params* __restr
     }
 }
 
-template <int V>
-__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k1_spmv_dot(const Params* __restrict__ dp, int s) {
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
+__global__ void __launch_bounds__(kThreads, 2) k1_spmv_dot(const Params* __restrict__ dp, int s) {
     __shared__ double sm[kWarps + 1];
     const Params P = *dp;
     if (P.scal->st[s].stop) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) P.scal->brk[s] = 0;
-    stream_smem_init<V>(dyn_smem);
-    uint32_t bits = 0;
-    const double d = phase_spmv<V, true>(P, P.p, P.q, blockIdx.x, gridDim.x, dyn_smem, bits);
+    const double d = phase_spmv_vector_dispatch<true>(P, P.p, P.q, blockIdx.x, gridDim.x);
     const double t = block_sum(d, sm);
     if (threadIdx.x == 0) P.part0[blockIdx.x] = t;
 }
@@ -202,19 +199,15 @@ __global__ void __launch_bounds__(kThreads, 2) k3_update_p(const Params* __restr
 // ---- loop mode 0: the whole solve as ONE cooperative persistent kernel.
 // Scalars live in registers, identical in every CTA; three grid barriers per
 // iteration (after K1, K2, K3); nothing leaves the device until the end.
-template <int V>
-__global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_persistent(Params P) {
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
+__global__ void __launch_bounds__(kThreads, 2) k_persistent(Params P) {
     __shared__ double sm[kWarps + 1];
     const int cta = blockIdx.x, G = gridDim.x;
     const bool lead = cta == 0 && threadIdx.x == 0;
     Scal* S = P.scal;
     unsigned long long epoch = 0;
-    uint32_t bits = 0;
-    stream_smem_init<V>(dyn_smem);
 
     // a0 prologue: q = A x0 ; r = b - q ; p = r ; rr, bb
-    phase_spmv<V, false>(P, P.x, P.q, cta, G, dyn_smem, bits);
+    phase_spmv_vector_dispatch<false>(P, P.x, P.q, cta, G);
     grid_barrier(&S->bar, G, epoch);
     phase_init_residual(P, cta, G, sm);
     grid_barrier(&S->bar, G, epoch);
@@ -227,38 +220,57 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<V>::value) k_persistent(Pa
     if (P.precond && S->diag_bad) { stop = 1; status = CG_BREAKDOWN; }
     if (lead && P.hist) P.hist[0] = sqrt(rr);
 
+    // Optional trace (cg_set_trace): thread 0 of every CTA stamps clock64 at 8 points of each
+    // of the first trace_iters iterations: 0 start, 1 K1 done, 2 past barrier 1, 3 K2 done,
+    // 4 past barrier 2, 5 beta known, 6 K3 done, 7 past barrier 3.
+    unsigned long long* tr = (P.trace && threadIdx.x == 0)
+        ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
+#define CG_STAMP(slot) do { if (tr && k < P.trace_iters) tr[k * kTraceSlots + (slot)] = clock64(); } while (0)
     while (!stop) {
+        CG_STAMP(0);
         // K1
-        const double d = phase_spmv<V, true>(P, P.p, P.q, cta, G, dyn_smem, bits);
+        const double d = phase_spmv_vector_dispatch<true>(P, P.p, P.q, cta, G);
         const double t = block_sum(d, sm);
         if (threadIdx.x == 0) P.part0[cta] = t;
+        CG_STAMP(1);
         grid_barrier(&S->bar, G, epoch);
+        CG_STAMP(2);
         // scalar alpha (every CTA, same order, same value)
         const double pq = sum_partials(P.part0, G, sm);
         if (!(pq > 0.0) || !is_finite(pq)) { stop = 1; status = CG_BREAKDOWN; break; }
         const double alpha = rz / pq;
         // K2
-        phase_update_xr<(V == 2 ? 4 : 2)>(P, alpha, cta, G, sm);
+        phase_update_xr<2>(P, alpha, cta, G, sm);
+        CG_STAMP(3);
         grid_barrier(&S->bar, G, epoch);
+        CG_STAMP(4);
         // scalar beta, continue-condition
         const double rr_new = sum_partials(P.part1, G, sm);
         const double rz_new = P.precond ? sum_partials(P.part2, G, sm) : rr_new;
         const double beta = rz_new / rz;
+        CG_STAMP(5);
         rr = rr_new; rz = rz_new; k += 1;
         const double res = sqrt(rr);
         if (lead && P.hist) P.hist[k] = res;
         if (res <= thresh) { stop = 1; status = CG_OK; break; }
         if (k >= P.maxit) { stop = 1; status = CG_MAXIT; break; }
+        k -= 1;
         // K3
-        phase_update_p<(V == 2 ? 4 : 2)>(P, beta, cta, G);
+        phase_update_p<2>(P, beta, cta, G);
+        CG_STAMP(6);
         grid_barrier(&S->bar, G, epoch);
+        CG_STAMP(7);
+        k += 1;
     }
+#undef CG_STAMP
     if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(rr); }
 }
 
 }  // namespace
 
 // ---------------------------------------------------------------- host side
+
+#include <stdio.h>
 
 static thread_local char g_cuda_err[256] = "no CUDA error recorded";
 
@@ -273,36 +285,78 @@ static thread_local char g_cuda_err[256] = "no CUDA error recorded";
         }                                                                     \
     } while (0)
 
-#include <stdio.h>
+// Streamed variants: W consumer warps, U entries in flight per lane (cg_stream.cuh).
+// "spmv" option value = index + 2.  W + kProducers is a multiple of 4 so the warps spread evenly
+// over the SM's four sub-partitions (their register files bound the registers per thread).
+struct StreamFns {
+    int W, U;
+    const void* spmv;
+    const void* init_spmv; const void* init_residual; const void* init_scalars;
+    const void* k1; const void* k2; const void* k3;
+    const void* persistent[3][2];          // [R index: 0 -> global vectors, 1 -> R = 2, 2 -> R = 4][Jacobi]
+};
+
+template <int W, int U> static StreamFns make_stream_fns() {
+    StreamFns f;
+    f.W = W; f.U = U;
+    f.spmv = (const void*)cgs::ks_spmv<W, U>;
+    f.init_spmv = (const void*)cgs::ks_init_spmv<W, U>;
+    f.init_residual = (const void*)cgs::ks_init_residual<W>;
+    f.init_scalars = (const void*)cgs::ks_init_scalars<W>;
+    f.k1 = (const void*)cgs::ks1_spmv_dot<W, U>;
+    f.k2 = (const void*)cgs::ks2_update_xr<W>;
+    f.k3 = (const void*)cgs::ks3_update_p<W>;
+    f.persistent[0][0] = (const void*)cgs::ks_persistent<W, U, 0, false>;
+    f.persistent[0][1] = (const void*)cgs::ks_persistent<W, U, 0, true>;
+    f.persistent[1][0] = (const void*)cgs::ks_persistent<W, U, 2, false>;
+    f.persistent[1][1] = (const void*)cgs::ks_persistent<W, U, 2, true>;
+    f.persistent[2][0] = (const void*)cgs::ks_persistent<W, U, 4, false>;
+    f.persistent[2][1] = (const void*)cgs::ks_persistent<W, U, 4, true>;
+    return f;
+}
+static constexpr int kNumStream = 3;
+static const StreamFns& stream_fns(int idx) {
+    static const StreamFns table[kNumStream] = {
+        make_stream_fns<12, 9>(), make_stream_fns<8, 27>(), make_stream_fns<8, 9>()};
+    return table[idx];
+}
 
 struct cg_handle {
     long long n, nnz;
     const int* rowptr; const int* colind; const double* vals;
     unsigned char* ws; size_t ws_bytes;
-    double *r, *p, *q, *dinv, *spare, *part0, *part1, *part2, *part3;
+    double *r, *p, *q, *dinv, *spare, *part0, *part1, *part2, *part3, *bslots;
+    int* rp_pad;
     Scal* scal; Params* dparams;
     Scal* h_scal; Params* h_params;        // pinned host mirrors
-    int sms;
-    int loop, spmv_opt, chunk, ctas_per_sm;
+    int sms, smem_optin;
+    size_t l2_bytes;
+    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead;
     int max_row_len, max_tile_nnz, tpr;
-    bool stream_ok, dinv_ready;
-    int grid_v[3];                         // cooperative grid per SpMV variant (index 1, 2)
+    bool dinv_ready;
+    int grid_generic;                      // cooperative grid of the generic variant
+    int cap, slots, slot_bytes;            // ring geometry of the streamed variants
+    bool stream_ok[kNumStream];
     cudaGraphExec_t gexec; int gexec_variant, gexec_chunk, gexec_grid;
     cudaStream_t cap_stream;               // capture-only stream (the legacy stream cannot capture)
+    unsigned long long* trace; int trace_iters;
     long long launches;
+    int last_resident;                     // R used by the last persistent solve (info)
 };
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static size_t vec_bytes(long long n) { return align_up((size_t)n * 8u, 256); }
+static size_t rp_pad_bytes(long long n) { return align_up((size_t)(n + 1 + cgs::kRpPad) * 4u, 256); }
 static constexpr int kNumVecs = 5;
 static constexpr size_t kPartBytes = (size_t)kMaxGrid * 8u;
+static constexpr size_t kBslotBytes = (size_t)cgs::kInboxStride * cgs::kBarGrid * 8u;    // one inbox per CTA
 static constexpr size_t kScalBytes = 512, kParamBytes = 512;
 
 extern "C" size_t cg_workspace_bytes(int64_t n) {
     if (n <= 0) return 0;
-    return kNumVecs * vec_bytes(n) + 4 * kPartBytes + kScalBytes + kParamBytes;
+    return kNumVecs * vec_bytes(n) + rp_pad_bytes(n) + 4 * kPartBytes + kBslotBytes + kScalBytes + kParamBytes;
 }
 
 extern "C" size_t cg_host_scratch_bytes(int64_t n, int64_t maxit) {
@@ -310,32 +364,56 @@ extern "C" size_t cg_host_scratch_bytes(int64_t n, int64_t maxit) {
     return 2 * vec_bytes(n) + align_up((size_t)(maxit + 1) * 8u, 256);
 }
 
-template <int V> static size_t variant_smem() { return V == 2 ? kStreamSmemBytes : 0; }
+static size_t stream_smem(const cg_handle* h) { return (size_t)h->slots * h->slot_bytes + cgs::kSmemTail; }
 
-template <int V> static int setup_variant(cg_handle* h) {
-    const size_t smem = variant_smem<V>();
-    if (smem) {
-        CK(cudaFuncSetAttribute(k_persistent<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_spmv<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_init_spmv<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k1_spmv_dot<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    }
+static int setup_generic(cg_handle* h) {
     int bps = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_persistent<V>, kThreads, smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_persistent, kThreads, 0));
     if (bps < 1) { snprintf(g_cuda_err, sizeof(g_cuda_err), "persistent kernel does not fit an SM"); return CG_ECUDA; }
-    int want = h->ctas_per_sm > 0 ? h->ctas_per_sm : (V == 2 ? 1 : 2);
+    int want = h->ctas_per_sm > 0 ? h->ctas_per_sm : 2;
     if (want > bps) want = bps;
     int g = h->sms * want;
     if (g > kMaxGrid) g = kMaxGrid;
-    h->grid_v[V] = g;
+    h->grid_generic = g;
     return CG_OK;
 }
 
+// Ring geometry from the matrix statistics, then per variant: does a ring of at least
+// W + 2 slots fit the opt-in shared memory?  (W slots may be held by consumers.)
+static int setup_stream(cg_handle* h) {
+    h->cap = (h->max_tile_nnz + 6 + 3) & ~3;
+    if (h->cap < 4) h->cap = 4;
+    h->slot_bytes = (int)align_up((size_t)h->cap * 12u + (size_t)cgs::kRpInts * 4u, 128);
+    const long long budget = (long long)h->smem_optin - cgs::kSmemTail;
+    long long S = budget / h->slot_bytes;
+    if (S > cgs::kMaxSlots) S = cgs::kMaxSlots;
+    // A slot must always be refilled by the same producer warp (tile j -> warp j mod kProducers,
+    // slot j mod S): otherwise a warp could run two phases ahead of a slot's "empty" barrier,
+    // which a parity wait cannot tell from zero phases ahead.
+    S -= S % cgs::kProducers;
+    h->slots = (int)S;
+    for (int v = 0; v < kNumStream; ++v) {
+        const StreamFns& f = stream_fns(v);
+        h->stream_ok[v] = S >= f.W + 2 && h->sms <= cgs::kBarGrid;
+        if (!h->stream_ok[v]) continue;
+        const int smem = h->smem_optin;      // the attribute is per function, not per handle: always the maximum
+        const void* fns[] = {f.spmv, f.init_spmv, f.init_residual, f.init_scalars, f.k1, f.k2, f.k3,
+                             f.persistent[0][0], f.persistent[0][1], f.persistent[1][0],
+                             f.persistent[1][1], f.persistent[2][0], f.persistent[2][1]};
+        for (const void* fn : fns)
+            CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    }
+    return CG_OK;
+}
+
+// 1 = generic; 2 + i = streamed variant i.
 static int pick_variant(const cg_handle* h) {
     if (h->spmv_opt == 1) return 1;
-    if (h->spmv_opt == 2) return h->stream_ok ? 2 : 1;
-    return h->stream_ok ? 2 : 1;
+    if (h->spmv_opt >= 2) return h->stream_ok[h->spmv_opt - 2] ? h->spmv_opt : 1;
+    return h->stream_ok[0] ? 2 : 1;
 }
+
+static int variant_grid(const cg_handle* h, int v) { return v == 1 ? h->grid_generic : h->sms; }
 
 static void fill_params(const cg_handle* h, Params* P, const double* b, double* x, double rtol,
                         long long maxit, double* hist, int precond, int variant) {
@@ -345,6 +423,11 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     P->part0 = h->part0; P->part1 = h->part1; P->part2 = h->part2; P->part3 = h->part3;
     P->scal = h->scal; P->hist = hist; P->rtol = rtol; P->maxit = maxit;
     P->precond = precond; P->spmv = variant; P->tpr = h->tpr;
+    P->trace = h->trace; P->trace_iters = h->trace_iters;
+    P->rp_pad = h->rp_pad; P->bslots = h->bslots;
+    P->cap = h->cap; P->slots = h->slots; P->slot_bytes = h->slot_bytes;
+    P->lookahead = h->lookahead;
+    P->l2_stream = ((size_t)h->nnz * 12u > h->l2_bytes / 2) ? 1 : 0;
 }
 
 extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
@@ -352,7 +435,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
                          size_t workspace_bytes) {
     if (!out) return CG_EINVAL;
     *out = nullptr;
-    if (n <= 0 || nnz < 0 || n >= (1LL << 31) - 1 || nnz >= (1LL << 31) - 8) return CG_EINVAL;
+    if (n <= 0 || nnz < 0 || n >= (1LL << 31) - 64 || nnz >= (1LL << 31) - 8) return CG_EINVAL;
     if (!d_rowptr || !d_workspace || (nnz > 0 && (!d_colind || !d_vals))) return CG_EINVAL;
     if (!aligned16(d_rowptr) || !aligned16(d_colind) || !aligned16(d_vals)) return CG_EINVAL;
     if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0) return CG_EINVAL;
@@ -377,12 +460,16 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     const size_t vb = vec_bytes(n);
     h->r = (double*)w; w += vb; h->p = (double*)w; w += vb; h->q = (double*)w; w += vb;
     h->dinv = (double*)w; w += vb; h->spare = (double*)w; w += vb;
+    h->rp_pad = (int*)w; w += rp_pad_bytes(n);
     h->part0 = (double*)w; w += kPartBytes; h->part1 = (double*)w; w += kPartBytes;
     h->part2 = (double*)w; w += kPartBytes; h->part3 = (double*)w; w += kPartBytes;
+    h->bslots = (double*)w; w += kBslotBytes;
     h->scal = (Scal*)w; w += kScalBytes; h->dparams = (Params*)w; w += kParamBytes;
     static_assert(sizeof(Scal) <= kScalBytes && sizeof(Params) <= kParamBytes, "workspace slots");
     h->sms = prop.multiProcessorCount;
-    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0;
+    h->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    h->l2_bytes = (size_t)prop.l2CacheSize;
+    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_params, sizeof(Params), cudaHostAllocDefault);
@@ -394,19 +481,20 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     }
 #define CKH(call) do { int rc_ = [&]() -> int { CK(call); return CG_OK; }(); \
         if (rc_ != CG_OK) { cg_destroy(h); return rc_; } } while (0)
-    // matrix statistics (one pass over rowptr on the legacy default stream)
+    // matrix statistics and the padded rowptr copy (legacy default stream)
     CKH(cudaMemsetAsync(h->scal, 0, sizeof(Scal), 0));
     k_stats<<<h->sms * 4, 256, 0, 0>>>(h->rowptr, h->n, h->scal);
+    CKH(cudaGetLastError());
+    k_pad_rowptr<<<h->sms * 4, 256, 0, 0>>>(h->rowptr, h->n, h->rp_pad, h->n + 1 + cgs::kRpPad);
     CKH(cudaGetLastError());
     CKH(cudaMemcpyAsync(h->h_scal, h->scal, sizeof(Scal), cudaMemcpyDeviceToHost, 0));
     CKH(cudaStreamSynchronize(0));
     h->max_row_len = h->h_scal->max_row_len;
     h->max_tile_nnz = h->h_scal->max_tile_nnz;
-    h->stream_ok = h->max_tile_nnz <= kTileCap;
     const double mean = (double)nnz / (double)n;
     h->tpr = mean <= 3 ? 2 : mean <= 6 ? 4 : mean <= 40 ? 8 : mean <= 96 ? 16 : 32;
-    int rc = setup_variant<1>(h);
-    if (rc == CG_OK) rc = setup_variant<2>(h);
+    int rc = setup_generic(h);
+    if (rc == CG_OK) rc = setup_stream(h);
     if (rc != CG_OK) { cg_destroy(h); return rc; }
     *out = h;
     return CG_OK;
@@ -437,8 +525,10 @@ extern "C" const char* cg_strerror(int code) {
 extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!h || !name) return CG_EINVAL;
     if (!strcmp(name, "loop")) { if (value < 0 || value > 2) return CG_EINVAL; h->loop = (int)value; return CG_OK; }
-    if (!strcmp(name, "spmv")) { if (value < 0 || value > 2) return CG_EINVAL; h->spmv_opt = (int)value; return CG_OK; }
+    if (!strcmp(name, "spmv")) { if (value < 0 || value > 1 + kNumStream) return CG_EINVAL; h->spmv_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "chunk")) { if (value < 2 || value > 4096 || (value & 1)) return CG_EINVAL; h->chunk = (int)value; return CG_OK; }
+    if (!strcmp(name, "lookahead")) { if (value < 0 || value > (1 << 30)) return CG_EINVAL; h->lookahead = (int)value; return CG_OK; }
+    if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "tpr")) {
         if (value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return CG_EINVAL;
         h->tpr = (int)value; return CG_OK;
@@ -446,11 +536,19 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!strcmp(name, "ctas_per_sm")) {
         if (value < 0 || value > 8) return CG_EINVAL;
         h->ctas_per_sm = (int)value;
-        int rc = setup_variant<1>(h);
-        if (rc == CG_OK) rc = setup_variant<2>(h);
-        return rc;
+        return setup_generic(h);
     }
     return CG_EINVAL;
+}
+
+// Rows per consumer thread the persistent kernel would keep in registers (0: global vectors).
+static int resident_rows(const cg_handle* h, int v) {
+    if (v < 2 || !h->resident_opt) return 0;
+    const long long ntiles = (h->n + kTileRows - 1) / kTileRows;
+    const long long tc_max = (ntiles + h->sms - 1) / h->sms;
+    const int W = stream_fns(v - 2).W;
+    const long long need = (tc_max + W - 1) / W;
+    return need <= 2 ? 2 : need <= 4 ? 4 : 0;
 }
 
 extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
@@ -458,16 +556,29 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     const int v = pick_variant(h);
     if (!strcmp(name, "loop")) *value = h->loop;
     else if (!strcmp(name, "spmv")) *value = v;
-    else if (!strcmp(name, "grid")) *value = h->grid_v[v];
-    else if (!strcmp(name, "block")) *value = kThreads;
-    else if (!strcmp(name, "smem")) *value = (int64_t)(v == 2 ? kStreamSmemBytes : 0);
+    else if (!strcmp(name, "grid")) *value = variant_grid(h, v);
+    else if (!strcmp(name, "block")) *value = v == 1 ? kThreads : 32 * (stream_fns(v - 2).W + cgs::kProducers);
+    else if (!strcmp(name, "smem")) *value = (int64_t)(v >= 2 ? stream_smem(h) : 0);
     else if (!strcmp(name, "launches")) *value = h->launches;
     else if (!strcmp(name, "sms")) *value = h->sms;
     else if (!strcmp(name, "tpr")) *value = h->tpr;
     else if (!strcmp(name, "max_row_len")) *value = h->max_row_len;
     else if (!strcmp(name, "max_tile_nnz")) *value = h->max_tile_nnz;
-    else if (!strcmp(name, "stream_ok")) *value = h->stream_ok ? 1 : 0;
+    else if (!strcmp(name, "stream_ok")) *value = h->stream_ok[0] ? 1 : 0;
+    else if (!strcmp(name, "consumer_warps")) *value = v >= 2 ? stream_fns(v - 2).W : 0;
+    else if (!strcmp(name, "in_flight")) *value = v >= 2 ? stream_fns(v - 2).U : 4;
+    else if (!strcmp(name, "ring_slots")) *value = v >= 2 ? h->slots : 0;
+    else if (!strcmp(name, "slot_bytes")) *value = v >= 2 ? h->slot_bytes : 0;
+    else if (!strcmp(name, "resident_rows")) *value = resident_rows(h, v);
     else return CG_EINVAL;
+    return CG_OK;
+}
+
+extern "C" int cg_set_trace(cg_handle* h, uint64_t* d_trace, int64_t iters) {
+    if (!h || iters < 0 || iters > (1 << 20) || (d_trace && (reinterpret_cast<uintptr_t>(d_trace) & 7u)))
+        return CG_EINVAL;
+    h->trace = (d_trace && iters > 0) ? reinterpret_cast<unsigned long long*>(d_trace) : nullptr;
+    h->trace_iters = h->trace ? (int)iters : 0;
     return CG_OK;
 }
 
@@ -489,8 +600,13 @@ extern "C" int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_
     const int v = pick_variant(h);
     Params P;
     fill_params(h, &P, nullptr, nullptr, 0.0, 0, nullptr, 0, v);
-    if (v == 2) k_spmv<2><<<h->grid_v[2], kThreads, kStreamSmemBytes, st>>>(P, d_x, d_y);
-    else        k_spmv<1><<<h->grid_v[1], kThreads, 0, st>>>(P, d_x, d_y);
+    if (v == 1) {
+        k_spmv<<<h->grid_generic, kThreads, 0, st>>>(P, d_x, d_y);
+    } else {
+        const StreamFns& f = stream_fns(v - 2);
+        void* args[] = {&P, &d_x, &d_y};
+        CK(cudaLaunchKernel(f.spmv, dim3(h->sms), dim3(32 * (f.W + cgs::kProducers)), args, stream_smem(h), st));
+    }
     CK(cudaGetLastError());
     h->launches = 1;
     return CG_OK;
@@ -512,48 +628,55 @@ extern "C" int cg_dot(cg_handle* h, const double* d_a, const double* d_b, double
     return CG_OK;
 }
 
-template <int V>
-static int launch_iteration_kernels(cg_handle* h, cudaStream_t st, int iters) {
-    const int G = h->grid_v[V];
-    const size_t smem = variant_smem<V>();
+// K1, K2, K3 of `iters` iterations as separate launches (captured into the graph of loop
+// mode 1, issued directly in loop mode 2).
+static int launch_iteration_kernels(cg_handle* h, int v, cudaStream_t st, int iters) {
+    const int G = variant_grid(h, v);
     for (int it = 0; it < iters; ++it) {
-        const int s = it & 1;
-        k1_spmv_dot<V><<<G, kThreads, smem, st>>>(h->dparams, s);
-        k2_update_xr<<<G, kThreads, 0, st>>>(h->dparams, s);
-        k3_update_p<<<G, kThreads, 0, st>>>(h->dparams, s);
+        int s = it & 1;
+        if (v == 1) {
+            k1_spmv_dot<<<G, kThreads, 0, st>>>(h->dparams, s);
+            k2_update_xr<<<G, kThreads, 0, st>>>(h->dparams, s);
+            k3_update_p<<<G, kThreads, 0, st>>>(h->dparams, s);
+        } else {
+            const StreamFns& f = stream_fns(v - 2);
+            const dim3 blk(32 * (f.W + cgs::kProducers));
+            const size_t smem = stream_smem(h);
+            void* args[] = {&h->dparams, &s};
+            CK(cudaLaunchKernel(f.k1, dim3(G), blk, args, smem, st));
+            CK(cudaLaunchKernel(f.k2, dim3(G), blk, args, smem, st));
+            CK(cudaLaunchKernel(f.k3, dim3(G), blk, args, smem, st));
+        }
     }
     CK(cudaGetLastError());
     return CG_OK;
 }
 
-template <int V>
-static int ensure_graph(cg_handle* h) {
-    if (h->gexec && h->gexec_variant == V && h->gexec_chunk == h->chunk && h->gexec_grid == h->grid_v[V])
+static int ensure_graph(cg_handle* h, int v) {
+    const int G = variant_grid(h, v);
+    if (h->gexec && h->gexec_variant == v && h->gexec_chunk == h->chunk && h->gexec_grid == G)
         return CG_OK;
     if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
     cudaGraph_t g = nullptr;
     if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    int rc = launch_iteration_kernels<V>(h, h->cap_stream, h->chunk);
+    int rc = launch_iteration_kernels(h, v, h->cap_stream, h->chunk);
     cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
     if (rc != CG_OK) { if (g) cudaGraphDestroy(g); return rc; }
     CK(e);
     e = cudaGraphInstantiate(&h->gexec, g, 0);
     cudaGraphDestroy(g);
     CK(e);
-    h->gexec_variant = V; h->gexec_chunk = h->chunk; h->gexec_grid = h->grid_v[V];
+    h->gexec_variant = v; h->gexec_chunk = h->chunk; h->gexec_grid = G;
     return CG_OK;
 }
 
-template <int V>
-static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol, long long maxit,
-                      double* d_hist, int precond, int64_t* h_iters, double* h_res,
-                      cudaStream_t st) {
-    const int G = h->grid_v[V];
-    const size_t smem = variant_smem<V>();
+static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, double rtol, long long maxit,
+                      double* d_hist, int precond, int64_t* h_iters, double* h_res, cudaStream_t st) {
+    const int G = variant_grid(h, v);
     h->launches = 0;
     if (precond && !h->dinv_ready) {
-        Params P; fill_params(h, &P, d_b, d_x, rtol, maxit, d_hist, precond, V);
+        Params P; fill_params(h, &P, d_b, d_x, rtol, maxit, d_hist, precond, v);
         CK(cudaMemsetAsync(&h->scal->diag_bad, 0, sizeof(int), st));
         k_diag_inv<<<h->sms * 4, 256, 0, st>>>(P);
         CK(cudaGetLastError());
@@ -562,19 +685,39 @@ static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol,
     }
     // zero the iteration state (everything before `check`), keep check / statistics
     CK(cudaMemsetAsync(h->scal, 0, offsetof(Scal, check), st));
-    fill_params(h, h->h_params, d_b, d_x, rtol, maxit, d_hist, precond, V);
+    fill_params(h, h->h_params, d_b, d_x, rtol, maxit, d_hist, precond, v);
 
     if (h->loop == 0) {
         Params P = *h->h_params;
         void* args[] = {&P};
-        CK(cudaLaunchCooperativeKernel((const void*)k_persistent<V>, dim3(G), dim3(kThreads), args, smem, st));
+        if (v == 1) {
+            CK(cudaLaunchCooperativeKernel((const void*)k_persistent, dim3(G), dim3(kThreads), args, 0, st));
+        } else {
+            const StreamFns& f = stream_fns(v - 2);
+            const int R = resident_rows(h, v);
+            const int ri = R == 2 ? 1 : R == 4 ? 2 : 0;
+            h->last_resident = R;
+            CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));        // arm the all-reduce slots
+            CK(cudaLaunchCooperativeKernel(f.persistent[ri][precond ? 1 : 0], dim3(G), dim3(32 * (f.W + cgs::kProducers)),
+                                           args, stream_smem(h), st));
+        }
         h->launches += 1;
     } else {
         CK(cudaMemcpyAsync(h->dparams, h->h_params, sizeof(Params), cudaMemcpyHostToDevice, st));
-        if (h->loop == 1) { int rc = ensure_graph<V>(h); if (rc != CG_OK) return rc; }
-        k_init_spmv<V><<<G, kThreads, smem, st>>>(h->dparams);
-        k_init_residual<<<G, kThreads, 0, st>>>(h->dparams);
-        k_init_scalars<<<G, kThreads, 0, st>>>(h->dparams);
+        if (h->loop == 1) { int rc = ensure_graph(h, v); if (rc != CG_OK) return rc; }
+        if (v == 1) {
+            k_init_spmv<<<G, kThreads, 0, st>>>(h->dparams);
+            k_init_residual<<<G, kThreads, 0, st>>>(h->dparams);
+            k_init_scalars<<<G, kThreads, 0, st>>>(h->dparams);
+        } else {
+            const StreamFns& f = stream_fns(v - 2);
+            const dim3 blk(32 * (f.W + cgs::kProducers));
+            const size_t smem = stream_smem(h);
+            void* args[] = {&h->dparams};
+            CK(cudaLaunchKernel(f.init_spmv, dim3(G), blk, args, smem, st));
+            CK(cudaLaunchKernel(f.init_residual, dim3(G), blk, args, smem, st));
+            CK(cudaLaunchKernel(f.init_scalars, dim3(G), blk, args, smem, st));
+        }
         CK(cudaGetLastError());
         h->launches += 3;
         while (true) {
@@ -582,7 +725,7 @@ static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol,
             CK(cudaStreamSynchronize(st));
             if (h->h_scal->st[0].stop) break;
             if (h->loop == 1) { CK(cudaGraphLaunch(h->gexec, st)); }
-            else { int rc = launch_iteration_kernels<V>(h, st, h->chunk); if (rc != CG_OK) return rc; }
+            else { int rc = launch_iteration_kernels(h, v, st, h->chunk); if (rc != CG_OK) return rc; }
             h->launches += 3LL * h->chunk;
         }
     }
@@ -598,10 +741,8 @@ static int solve_checked(cg_handle* h, const double* d_b, double* d_x, double rt
     if (!h || !d_b || !d_x || d_b == d_x) return CG_EINVAL;
     if (!(rtol >= 0.0) || maxit < 0) return CG_EINVAL;          // also rejects NaN
     if (!aligned16(d_b) || !aligned16(d_x) || (reinterpret_cast<uintptr_t>(d_hist) & 7u)) return CG_EINVAL;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (pick_variant(h) == 2)
-        return solve_impl<2>(h, d_b, d_x, rtol, maxit, d_hist, precond, h_iters, h_res, st);
-    return solve_impl<1>(h, d_b, d_x, rtol, maxit, d_hist, precond, h_iters, h_res, st);
+    return solve_impl(h, pick_variant(h), d_b, d_x, rtol, maxit, d_hist, precond, h_iters, h_res,
+                      static_cast<cudaStream_t>(stream));
 }
 
 extern "C" int cg_solve(cg_handle* h, const double* d_b, double* d_x, double rtol, int64_t maxit,

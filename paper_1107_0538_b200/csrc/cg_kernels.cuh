@@ -23,16 +23,7 @@ namespace cgk {
 constexpr int kThreads = 256;       // threads per CTA, every kernel
 constexpr int kWarps = kThreads / 32;
 constexpr int kMaxGrid = 2048;
-// ptxas schedules for ILP only when told the occupancy target: 1 CTA/SM for the streamed
-// variant (shared-memory bound anyway), 2 for the sub-warp variant.
-template <int V> struct MinBlocks { static constexpr int value = (V == 2) ? 1 : 2; };      // capacity of each partials array
-
-// SpMV variant B (bulk-async streamed tiles): each warp owns a private ring of
-// kStages tiles of kTileRows rows; a tile's nnz span must fit kTileCap entries.
-constexpr int kTileRows = 32;
-constexpr int kTileCap = 1016;      // nnz per tile (<= 31.75 per row on average)
-constexpr int kTileBuf = kTileCap + 8;   // + up to 3 entries of widening at each end, padded
-constexpr int kStages = 2;
+constexpr int kTileRows = 32;       // rows per tile of the streamed SpMV (one lane per row)
 
 struct State {            // one per iteration parity (loop modes 1, 2)
     double rr;            // ||r_k||^2
@@ -78,9 +69,21 @@ struct Params {
     double rtol;
     long long maxit;
     int precond;          // 0 none (the paper's path), 1 Jacobi
-    int spmv;             // 1 vector, 2 stream
+    int spmv;             // 1 sub-warp per row from global, >= 2 streamed (cg_stream.cuh)
     int tpr;              // lanes per row of the vector variant
+    unsigned long long* trace;   // optional phase stamps of the persistent kernel (cg_set_trace)
+    int trace_iters;
+    // streamed variants (cg_stream.cuh)
+    const int* rp_pad;    // rowptr copied into the workspace, padded with nnz (bulk copies of 36 ints)
+    double* bslots;       // grid all-reduce inboxes [cta][3][kBarVals][kBarGrid], all-ones when idle
+    int cap;              // entries per ring slot (multiple of 4)
+    int slots;            // ring depth S
+    int slot_bytes;       // cap * 12 + 144, rounded up to 128
+    int lookahead;        // producer run-ahead (tiles) into a pass the consumers have not started
+    int l2_stream;        // 1: the matrix does not fit the L2 -> evict-first hint on its copies
 };
+
+constexpr int kTraceSlots = 16;  // stamps per iteration and CTA, see k_persistent
 
 // ---------------------------------------------------------------- small helpers
 
@@ -215,18 +218,7 @@ __device__ __forceinline__ double phase_spmv_vector_dispatch(const Params& P, co
     }
 }
 
-// ---------------------------------------------------------------- K1, variant B
-// Bulk-async (TMA, cp.async.bulk -> SASS UBLKCP) streaming of the contiguous
-// vals/colind span of a 32-row tile into a warp-private shared-memory ring, then
-// one thread per row walks its entries out of shared memory.  For the natural-
-// ordered stencil the x gathers of the 32 lanes are consecutive addresses.
-//
-// Alignment: cp.async.bulk needs 16-byte aligned source, destination and size.
-// The span [s, e) of a tile is widened to [s & ~3, ...) so both the int32 and the
-// fp64 source addresses are 16-byte aligned (the arrays themselves are, by the
-// cg_create contract); the end is rounded up but clamped to nnz rounded DOWN to a
-// multiple of 4, and the <= 3 trailing entries of the whole matrix are fetched
-// with ordinary loads, so nothing outside the arrays is ever touched.
+// ---------------------------------------------------------------- mbarrier / bulk-copy primitives
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return (uint32_t)__cvta_generic_to_shared(p);
 }
@@ -256,121 +248,18 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
         " [%0], [%1], %2, [%3], %4;"
         :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
 }
+__device__ __forceinline__ void bulk_g2s_plain(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
-}
-
-struct __align__(16) WarpStage {
-    double vals[kTileBuf];
-    int cols[kTileBuf];
-};
-struct StreamSmem {
-    WarpStage stage[kWarps][kStages];
-    uint64_t full[kWarps][kStages];
-};
-constexpr size_t kStreamSmemBytes = sizeof(StreamSmem);
-
-// Issue the copies for tile `t` into `st` (called by lane 0 of the owning warp).
-// Returns nothing; the span base (first fetched entry index) is recomputed by readers.
-__device__ __forceinline__ void stream_issue(const Params& P, long long t, WarpStage* st,
-                                             uint64_t* bar, uint64_t policy) {
-    const long long row0 = t * kTileRows;
-    const long long row1 = (row0 + kTileRows < P.n) ? row0 + kTileRows : P.n;
-    const int s = __ldg(P.rowptr + row0), e = __ldg(P.rowptr + row1);
-    const int s4 = s & ~3;
-    const int lim = (int)(P.nnz & ~3LL);              // last entry reachable by bulk copies
-    int e4 = (e + 3) & ~3;
-    if (e4 > lim) e4 = lim;
-    const int cnt = e4 > s4 ? e4 - s4 : 0;            // multiple of 4
-    if (cnt > 0) {
-        mbar_expect_tx(bar, (uint32_t)cnt * 12u);
-        bulk_g2s(st->vals, P.vals + s4, (uint32_t)cnt * 8u, bar, policy);
-        bulk_g2s(st->cols, P.colind + s4, (uint32_t)cnt * 4u, bar, policy);
-    } else {
-        mbar_expect_tx(bar, 0u);
-    }
-}
-
-template <bool DOT>
-__device__ __forceinline__ double phase_spmv_stream(const Params& P, const double* x, double* y,
-                                                    int cta, int G, StreamSmem* sm,
-                                                    uint32_t& phase_bits) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const long long ntiles = (P.n + kTileRows - 1) / kTileRows;
-    const long long gw = (long long)cta * kWarps + warp;          // global warp id
-    const long long nw = (long long)G * kWarps;
-    const uint64_t policy = l2_policy_evict_first();
-    const int lim = (int)(P.nnz & ~3LL);
-    double dot = 0.0;
-
-    // prime the ring
-    if (lane == 0) {
-#pragma unroll
-        for (int sidx = 0; sidx < kStages; ++sidx) {
-            const long long t = gw + (long long)sidx * nw;
-            if (t < ntiles) stream_issue(P, t, &sm->stage[warp][sidx], &sm->full[warp][sidx], policy);
-        }
-    }
-    int sidx = 0;
-    for (long long t = gw; t < ntiles; t += nw) {
-        WarpStage* st = &sm->stage[warp][sidx];
-        const long long row = t * kTileRows + lane;
-        const long long rlast = (t * kTileRows + kTileRows < P.n) ? t * kTileRows + kTileRows : P.n;
-        const int tile_s = __ldg(P.rowptr + t * kTileRows);
-        const int tile_e = __ldg(P.rowptr + rlast);
-        const int base = tile_s & ~3;
-        int s = 0, e = 0;
-        if (row < P.n) { s = __ldg(P.rowptr + row); e = __ldg(P.rowptr + row + 1); }
-        // trailing <= 3 entries of the matrix that no bulk copy may cover
-        if (tile_e > lim) {
-            const int k = lim + lane;
-            if (lane < 4 && k < tile_e && k >= base) {
-                st->vals[k - base] = ld_stream_f64(P.vals + k);
-                st->cols[k - base] = ld_stream_s32(P.colind + k);
-            }
-        }
-        mbar_wait(&sm->full[warp][sidx], (phase_bits >> sidx) & 1u);
-        phase_bits ^= (1u << sidx);
-        __syncwarp();
-        // kUnroll entries per trip: all shared-memory reads first, then all x gathers, then
-        // the FMAs into 3 independent accumulators (27 = 3 x 9 for the stencil rows).
-        constexpr int kUnroll = 9;
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-        const int ks = s - base, ke = e - base;
-        for (int k = ks; k < ke; k += kUnroll) {
-            double v[kUnroll];
-            int c[kUnroll];
-#pragma unroll
-            for (int u = 0; u < kUnroll; ++u) {
-                const bool ok = k + u < ke;
-                const int kk = ok ? k + u : ke - 1;          // stay inside this row's span
-                c[u] = st->cols[kk];
-                v[u] = ok ? st->vals[kk] : 0.0;
-            }
-            double xv[kUnroll];
-#pragma unroll
-            for (int u = 0; u < kUnroll; ++u) xv[u] = ld_global_f64(x + c[u]);
-#pragma unroll
-            for (int u = 0; u < kUnroll; u += 3) {
-                a0 = fma(v[u], xv[u], a0);
-                a1 = fma(v[u + 1], xv[u + 1], a1);
-                a2 = fma(v[u + 2], xv[u + 2], a2);
-            }
-        }
-        const double acc = (a0 + a1) + a2;
-        if (row < P.n) {
-            y[row] = acc;
-            if (DOT) dot = fma(acc, x[row], dot);
-        }
-        __syncwarp();                      // every lane is done reading this stage
-        const long long tn = t + (long long)kStages * nw;
-        if (lane == 0 && tn < ntiles)
-            stream_issue(P, tn, st, &sm->full[warp][sidx], policy);
-        sidx = (sidx + 1 == kStages) ? 0 : sidx + 1;
-    }
-    return dot;
 }
 
 // ---------------------------------------------------------------- vector phases
@@ -505,29 +394,6 @@ __device__ __forceinline__ void phase_update_p(const Params& P, double beta, int
 __device__ __forceinline__ void phase_zero_x(const Params& P, int cta, int G) {
     const long long stride = (long long)G * kThreads;
     for (long long i = (long long)cta * kThreads + threadIdx.x; i < P.n; i += stride) P.x[i] = 0.0;
-}
-
-// One SpMV phase.  VARIANT 1 = sub-warp per row from global, 2 = streamed tiles.
-template <int VARIANT, bool DOT>
-__device__ __forceinline__ double phase_spmv(const Params& P, const double* x, double* y, int cta,
-                                             int G, unsigned char* dyn_smem, uint32_t& phase_bits) {
-    if constexpr (VARIANT == 2)
-        return phase_spmv_stream<DOT>(P, x, y, cta, G, reinterpret_cast<StreamSmem*>(dyn_smem),
-                                      phase_bits);
-    else
-        return phase_spmv_vector_dispatch<DOT>(P, x, y, cta, G);
-}
-
-template <int VARIANT>
-__device__ __forceinline__ void stream_smem_init(unsigned char* dyn_smem) {
-    if constexpr (VARIANT == 2) {
-        StreamSmem* sm = reinterpret_cast<StreamSmem*>(dyn_smem);
-        if (threadIdx.x < kWarps * kStages)
-            mbar_init(&sm->full[threadIdx.x / kStages][threadIdx.x % kStages], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncthreads();
-    }
 }
 
 }  // namespace cgk

@@ -1,0 +1,328 @@
+// cg_stream_kernels.cuh -- kernel entry points of the streamed CG path (see cg_stream.cuh).
+// Every kernel is launched with 32 (W + kProducers) threads: W consumer warps and the producer
+// warps, which return at once in kernels that do not stream the matrix.
+#pragma once
+#include "cg_stream.cuh"
+#include "../../include/cg.h"
+#include <limits.h>
+
+namespace cgs {
+
+__device__ __forceinline__ bool finite_d(double v) { return fabs(v) <= 1.79769313486231570e308; }
+
+// Everything the loop decides from (rr, bb) before the first iteration.
+__device__ __forceinline__ void decide_start(const Params& P, double rr, double bb, int* stop,
+                                             int* status, double* thresh) {
+    *thresh = P.rtol * sqrt(bb);
+    *stop = 0; *status = CG_OK;
+    if (bb == 0.0 || sqrt(rr) <= *thresh) { *stop = 1; *status = CG_OK; }
+    else if (P.maxit <= 0) { *stop = 1; *status = CG_MAXIT; }
+}
+
+#define CGS_PROLOGUE(W)                                                         \
+    extern __shared__ __align__(128) unsigned char dyn[];                       \
+    Ring rg = ring_view(P, dyn);                                                \
+    const int cta = blockIdx.x, G = gridDim.x;                                  \
+    const int warp = threadIdx.x >> 5;                                          \
+    long long tb; int Tc;                                                       \
+    cta_tiles(P, cta, G, tb, Tc);                                               \
+    (void)warp
+
+// ---- cg_spmv: y = A x
+template <int W, int U>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_spmv(Params P, const double* x, double* y) {
+    CGS_PROLOGUE(W);
+    ring_init(rg);
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
+    phase_spmv_tiles<W, U, false>(P, rg, x, y, tb, Tc, RingPos{0u, 0u});
+}
+
+// ---- stand-alone kernels of loop modes 1 (graph) and 2 (stepwise).  They read Params from
+// ---- device memory so that a captured graph survives across solves.
+
+template <int W, int U>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_spmv(const Params* __restrict__ dp) {
+    const Params P = *dp;
+    CGS_PROLOGUE(W);
+    ring_init(rg);
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
+    phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, RingPos{0u, 0u});
+}
+
+template <int W>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_residual(const Params* __restrict__ dp) {
+    const Params P = *dp;
+    CGS_PROLOGUE(W);
+    if (warp >= W) return;
+    double arr = 0.0, abb = 0.0, arz = 0.0;
+    if (P.precond) phase_init_tiles<W, true>(P, tb, Tc, arr, abb, arz);
+    else           phase_init_tiles<W, false>(P, tb, Tc, arr, abb, arz);
+    double t = block_sum_w<W>(arr, rg.red); if (threadIdx.x == 0) P.part1[cta] = t;
+    t = block_sum_w<W>(abb, rg.red);        if (threadIdx.x == 0) P.part2[cta] = t;
+    if (P.precond) { t = block_sum_w<W>(arz, rg.red); if (threadIdx.x == 0) P.part3[cta] = t; }
+}
+
+template <int W>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_scalars(const Params* __restrict__ dp) {
+    const Params P = *dp;
+    CGS_PROLOGUE(W);
+    if (warp >= W) return;
+    double rr = sum_partials_w<W>(P.part1, G, rg.red);
+    const double bb = sum_partials_w<W>(P.part2, G, rg.red);
+    const double rz = P.precond ? sum_partials_w<W>(P.part3, G, rg.red) : rr;
+    if (bb == 0.0) { phase_zero_x_tiles<W>(P, tb, Tc); rr = 0.0; }
+    if (cta == 0 && threadIdx.x == 0) {
+        int stop, status; double thresh;
+        decide_start(P, rr, bb, &stop, &status, &thresh);
+        if (P.precond && P.scal->diag_bad) { stop = 1; status = CG_BREAKDOWN; }
+        Scal* S = P.scal;
+        S->bb = bb; S->thresh = thresh;
+        S->st[0].rr = rr; S->st[0].rz = rz; S->st[0].k = 0; S->st[0].stop = stop; S->st[0].status = status;
+        if (P.hist) P.hist[0] = sqrt(rr);
+        S->out_iters = 0; S->out_status = status; S->out_res = sqrt(rr);
+    }
+}
+
+template <int W, int U>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks1_spmv_dot(const Params* __restrict__ dp, int s) {
+    const Params P = *dp;
+    if (P.scal->st[s].stop) return;
+    CGS_PROLOGUE(W);
+    if (cta == 0 && threadIdx.x == 0) P.scal->brk[s] = 0;
+    ring_init(rg);
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
+    const double d = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, RingPos{0u, 0u});
+    const double t = block_sum_w<W>(d, rg.red);
+    if (threadIdx.x == 0) P.part0[cta] = t;
+}
+
+template <int W>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks2_update_xr(const Params* __restrict__ dp, int s) {
+    const Params P = *dp;
+    if (P.scal->st[s].stop) return;
+    CGS_PROLOGUE(W);
+    if (warp >= W) return;
+    const double pq = sum_partials_w<W>(P.part0, G, rg.red);
+    if (!(pq > 0.0) || !finite_d(pq)) {
+        if (cta == 0 && threadIdx.x == 0) P.scal->brk[s] = 1;
+        return;
+    }
+    const double alpha = P.scal->st[s].rz / pq;
+    double arr = 0.0, arz = 0.0;
+    if (P.precond) phase_xr_tiles<W, true>(P, alpha, tb, Tc, arr, arz);
+    else           phase_xr_tiles<W, false>(P, alpha, tb, Tc, arr, arz);
+    double t = block_sum_w<W>(arr, rg.red); if (threadIdx.x == 0) P.part1[cta] = t;
+    if (P.precond) { t = block_sum_w<W>(arz, rg.red); if (threadIdx.x == 0) P.part2[cta] = t; }
+}
+
+template <int W>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks3_update_p(const Params* __restrict__ dp, int s) {
+    const Params P = *dp;
+    CGS_PROLOGUE(W);
+    if (warp >= W) return;
+    Scal* S = P.scal;
+    const State st = S->st[s];
+    const bool lead = cta == 0 && threadIdx.x == 0;
+    if (st.stop) { if (lead) S->st[s ^ 1] = st; return; }
+    if (S->brk[s]) {
+        if (lead) {
+            State nx = st; nx.stop = 1; nx.status = CG_BREAKDOWN;
+            S->st[s ^ 1] = nx;
+            S->out_iters = st.k; S->out_status = CG_BREAKDOWN; S->out_res = sqrt(st.rr);
+        }
+        return;
+    }
+    const double rr = sum_partials_w<W>(P.part1, G, rg.red);
+    const double rz = P.precond ? sum_partials_w<W>(P.part2, G, rg.red) : rr;
+    const double beta = rz / st.rz;
+    const long long k = st.k + 1;
+    const double res = sqrt(rr);
+    int stop = 0, status = CG_OK;
+    if (res <= S->thresh) { stop = 1; status = CG_OK; }
+    else if (k >= P.maxit) { stop = 1; status = CG_MAXIT; }
+    if (lead) {
+        State nx; nx.rr = rr; nx.rz = rz; nx.k = k; nx.stop = stop; nx.status = status;
+        S->st[s ^ 1] = nx;
+        if (P.hist) P.hist[k] = res;
+        if (stop) { S->out_iters = k; S->out_status = status; S->out_res = res; }
+    }
+    if (!stop) {
+        if (P.precond) phase_p_tiles<W, true>(P, beta, tb, Tc);
+        else           phase_p_tiles<W, false>(P, beta, tb, Tc);
+    }
+}
+
+// ---- loop mode 0: the whole solve as ONE cooperative persistent kernel.
+// R > 0: every consumer thread owns at most R rows (tiles warp, warp + W, ...) and keeps
+//        x, r, p, q (and D^-1) of those rows in registers from the prologue to the end; the
+//        only vector traffic left per iteration is the store of p and the gathers of K1.
+// R = 0: vectors in global memory (systems with more than R_max * 32 * W * G rows).
+// Scalars live in registers, identical in every CTA; three grid all-reduces per iteration
+// (after K1: p.q; after K2: r.r; after K3: a pure barrier that publishes p).
+template <int W, int U, int R, bool PRE>
+__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P) {
+    CGS_PROLOGUE(W);
+    ring_init(rg);
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, LLONG_MAX, warp - W, kProducers); return; }
+    const int lane = threadIdx.x & 31;
+    const bool lead = cta == 0 && threadIdx.x == 0;
+    Scal* S = P.scal;
+    unsigned bcount = 0;
+    unsigned long long pass = 0;
+    RingPos pos{0u, 0u};
+    constexpr int RR = R > 0 ? R : 1;
+    double xr[RR], rv[RR], pv[RR], qv[RR], dv[RR];
+    long long row[RR];
+
+    // a0 prologue: q = A x0 ; r = b - q ; p = r ; rr, bb
+    double arr = 0.0, abb = 0.0, arz = 0.0;
+    consumers_begin_pass(rg, pass);
+    if constexpr (R > 0) {
+        double bv[RR];
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            const int j = warp + kk * W;
+            const long long i = (tb + j) * kTileRows + lane;
+            row[kk] = (j < Tc && i < P.n) ? i : -1;
+            xr[kk] = 0.0; bv[kk] = 0.0; dv[kk] = 1.0; qv[kk] = 0.0; rv[kk] = 0.0; pv[kk] = 0.0;
+            if (row[kk] >= 0) { xr[kk] = P.x[i]; bv[kk] = P.b[i]; if (PRE) dv[kk] = P.dinv[i]; }
+        }
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            const int j = warp + kk * W;
+            if (j < Tc) qv[kk] = consume_tile<U>(rg, P.x, pos, j, lane);
+        }
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            if (row[kk] < 0) continue;
+            const double ri = bv[kk] - qv[kk];
+            rv[kk] = ri;
+            abb = fma(bv[kk], bv[kk], abb);
+            arr = fma(ri, ri, arr);
+            if (PRE) { const double zi = dv[kk] * ri; pv[kk] = zi; arz = fma(ri, zi, arz); }
+            else pv[kk] = ri;
+            P.p[row[kk]] = pv[kk];
+        }
+    } else {
+        phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, pos);
+        phase_init_tiles<W, PRE>(P, tb, Tc, arr, abb, arz);     // reads only this thread's own q
+    }
+    ++pass; pos = ring_advance(rg, pos, (unsigned)Tc);
+    double rr, bb, rz;
+    {
+        double v[PRE ? 3 : 2];
+        v[0] = arr; v[1] = abb;
+        if (PRE) v[PRE ? 2 : 0] = arz;
+        grid_allreduce<W, (PRE ? 3 : 2), true>(P, rg.red, bcount, cta, G, v);
+        rr = v[0]; bb = v[1]; rz = PRE ? v[PRE ? 2 : 0] : rr;
+    }
+    if (bb == 0.0) {
+        if constexpr (R > 0) {
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) xr[kk] = 0.0;
+        } else {
+            phase_zero_x_tiles<W>(P, tb, Tc);
+        }
+        rr = 0.0;
+    }
+    long long k = 0; int stop, status; double thresh;
+    decide_start(P, rr, bb, &stop, &status, &thresh);
+    if (PRE && S->diag_bad) { stop = 1; status = CG_BREAKDOWN; }
+    if (lead && P.hist) P.hist[0] = sqrt(rr);
+
+    // Optional trace (cg_set_trace): thread 0 of every CTA stamps clock64 at 8 points of each
+    // of the first trace_iters iterations: 0 start, 1 K1 done, 2 past all-reduce 1, 3 K2 done,
+    // 4 past all-reduce 2, 5 beta known, 6 K3 done, 7 past barrier 3.
+    unsigned long long* tr = (P.trace && threadIdx.x == 0)
+        ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
+    unsigned long long full_wait = 0;
+    if (tr) rg.acc = &full_wait;
+#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
+    while (!stop) {
+        CGS_STAMP(k, 0);
+        // K1: q = A p, partial p.q
+        double dot = 0.0;
+        consumers_begin_pass(rg, pass);
+        if constexpr (R > 0) {
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) {
+                const int j = warp + kk * W;
+                if (j < Tc) {
+                    qv[kk] = consume_tile<U>(rg, P.p, pos, j, lane);
+                    if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                }
+            }
+        } else {
+            dot = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, pos);
+        }
+        ++pass; pos = ring_advance(rg, pos, (unsigned)Tc);
+        CGS_STAMP(k, 1);
+        double v1[1] = {dot};
+        grid_allreduce<W, 1, false>(P, rg.red, bcount, cta, G, v1);
+        CGS_STAMP(k, 2);
+        // scalar alpha (every CTA, same order, same value)
+        const double pq = v1[0];
+        if (!(pq > 0.0) || !finite_d(pq)) { stop = 1; status = CG_BREAKDOWN; break; }
+        const double alpha = rz / pq;
+        // K2: x += alpha p ; r -= alpha q ; partial r.r
+        arr = 0.0; arz = 0.0;
+        if constexpr (R > 0) {
+            const double na = -alpha;
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) {
+                if (row[kk] < 0) continue;
+                xr[kk] = fma(alpha, pv[kk], xr[kk]);
+                rv[kk] = fma(na, qv[kk], rv[kk]);
+                arr = fma(rv[kk], rv[kk], arr);
+                if (PRE) arz = fma(rv[kk], dv[kk] * rv[kk], arz);
+            }
+        } else {
+            phase_xr_tiles<W, PRE>(P, alpha, tb, Tc, arr, arz);
+        }
+        CGS_STAMP(k, 3);
+        double v2[PRE ? 2 : 1];
+        v2[0] = arr;
+        if (PRE) v2[PRE ? 1 : 0] = arz;
+        grid_allreduce<W, (PRE ? 2 : 1), false>(P, rg.red, bcount, cta, G, v2);
+        CGS_STAMP(k, 4);
+        // scalar beta, continue-condition
+        const double rr_new = v2[0];
+        const double rz_new = PRE ? v2[PRE ? 1 : 0] : rr_new;
+        const double beta = rz_new / rz;
+        rr = rr_new; rz = rz_new;
+        const double res = sqrt(rr);
+        CGS_STAMP(k, 5);
+        k += 1;
+        if (lead && P.hist) P.hist[k] = res;
+        if (res <= thresh) { stop = 1; status = CG_OK; break; }
+        if (k >= P.maxit) { stop = 1; status = CG_MAXIT; break; }
+        // K3: p = r + beta p
+        if constexpr (R > 0) {
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) {
+                if (row[kk] < 0) continue;
+                const double zi = PRE ? rv[kk] * dv[kk] : rv[kk];
+                pv[kk] = fma(beta, pv[kk], zi);
+                P.p[row[kk]] = pv[kk];
+            }
+        } else {
+            phase_p_tiles<W, PRE>(P, beta, tb, Tc);
+        }
+        CGS_STAMP(k - 1, 6);
+        double v0[1] = {0.0};
+        grid_allreduce<W, 1, true>(P, rg.red, bcount, cta, G, v0,       // publishes p
+                              (tr && k - 1 < P.trace_iters) ? tr + (k - 1) * kTraceSlots + 8 : nullptr);
+        CGS_STAMP(k - 1, 7);
+    }
+#undef CGS_STAMP
+    if constexpr (R > 0) {
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk)
+            if (row[kk] >= 0) P.x[row[kk]] = xr[kk];
+    }
+    if (tr) tr[(size_t)P.trace_iters * kTraceSlots + 3] = full_wait;
+    if (threadIdx.x == 0) consumers_stop(rg, pass);
+    if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(rr); }
+}
+
+}  // namespace cgs
