@@ -101,6 +101,23 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def describe(A):
+    """Launch configuration of a bound handle, from cg_get_info."""
+    v = A.info("spmv")
+    d = {"loop": {0: "persistent cooperative kernel", 1: "cuda graph", 2: "stepwise launches"}[A.info("loop")],
+         "grid": A.info("grid"), "block": A.info("block"), "smem_bytes": A.info("smem")}
+    if v == 1:
+        d["spmv"] = f"generic: {A.info('tpr')} lanes per row from global memory"
+    else:
+        d["spmv"] = (f"streamed: 4 TMA producer warps + {A.info('consumer_warps')} consumer warps, one lane per row, "
+                     f"{A.info('in_flight')} gathers in flight per lane, ring of {A.info('ring_slots')} x "
+                     f"{A.info('slot_bytes')} B tiles")
+        rr = A.info("resident_rows")
+        d["vectors"] = (f"x, r, p, q in registers ({rr} rows per thread)" if rr and A.info("loop") == 0
+                        else "x, r, p, q in global memory")
+    return d
+
+
 def time_oracle(problem, seconds_budget, fixed_iters=None):
     """The CPU oracle as it stands, single thread, on a bounded sample of the workload."""
     from oracle import cg_oracle as orc
@@ -165,6 +182,7 @@ def main():
     ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--lookahead", type=int, default=None)
     ap.add_argument("--resident", type=int, default=None)
+    ap.add_argument("--ring-slots", type=int, default=None)
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -229,6 +247,8 @@ def main():
             Ap.set_option("lookahead", args.lookahead)
         if args.resident is not None:
             Ap.set_option("resident", args.resident)
+        if args.ring_slots is not None:
+            Ap.set_option("ring_slots", args.ring_slots)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []
@@ -337,6 +357,12 @@ def main():
     h2d = 2 * 8 * p.n
     d2h = 8 * p.n + 8 * (e2e_it // args.steps + 1) + 192
 
+    # measured read rooflines on this box (cg_probe_read_bandwidth): 40 MB sweeps stay in the L2,
+    # 2 GiB sweeps come from HBM
+    l2_gbs = A.probe_read_bandwidth(40 << 20, reps=50)
+    hbm_read_gbs = A.probe_read_bandwidth(2 << 30, reps=5)
+    t_iter = t_dev / iters_total if world == 1 else None
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True,
@@ -347,9 +373,7 @@ def main():
             "iterations_per_solve": it_per_solve,
             "l2": "flushed (512 MiB write) between steps, outside the timed event pairs; inside a solve the "
                   "41.9 MB CSR matrix is L2-resident by design",
-            "loop": {0: "persistent cooperative kernel", 1: "cuda graph", 2: "stepwise launches"}[A.info("loop")],
-            "spmv": {1: "sub-warp per row", 2: "bulk-async streamed tiles"}[A.info("spmv")],
-            "grid": A.info("grid"), "block": A.info("block"), "smem_bytes": A.info("smem"),
+            **describe(A),
             "parallelism": "replicas only (north_star: one GPU, no sharding, no collectives)",
         },
         "us_per_iteration": t_dev / iters_total * 1e6 if world == 1 else None,
@@ -369,6 +393,12 @@ def main():
             "note": "working set 53.5 MB is L2-resident: this config is bound by L2 bandwidth and grid-sync "
                     "latency, the HBM fraction is reported as north_star asks; see north_star_160 for the HBM-bound case",
         },
+        "roofline_l2": {"bound": "l2", "achieved": bytes_it / t_iter / 1e9 if t_iter else None, "peak": l2_gbs,
+                        "unit": "GB/s", "frac": (bytes_it / t_iter / 1e9 / l2_gbs) if t_iter else None,
+                        "peak_source": "measured here: cg_probe_read_bandwidth over a 40 MiB buffer (L2-resident), 50 sweeps",
+                        "hbm_read_gbs_measured_here": hbm_read_gbs,
+                        "us_per_iteration": t_iter * 1e6 if t_iter else None,
+                        "us_at_l2_peak": bytes_it / l2_gbs / 1e3, "us_at_hbm_peak": bytes_it / peak / 1e3},
         "paper_context": {"source": "PAPER.md:52-57 Table I (Tesla T10 / Core 2 Duo, the paper's own FEM matrix)",
                           "opencl_1gpu_iters_per_s": 116 / 0.659, "matlab_pcg_iters_per_s": 117 / 3.17,
                           "opencl_4gpu_iters_per_s": 116 / 0.380},
@@ -408,6 +438,7 @@ def main():
                 "roofline": {"bound": "hbm", "achieved": gbs4, "peak": peak, "unit": "GB/s",
                              "frac": gbs4 / peak, "traffic": None, "target_frac": 0.70},
                 "cg_gflops": cg_inputs.flops_per_iteration(p4.n, p4.nnz) * K / t4 / 1e9,
+                "launch": describe(A4),
             }
             A4.close()
             del b4, x4, A4

@@ -48,14 +48,16 @@ typedef struct cg_handle cg_handle;
 #define CG_EUNSUPPORTED  -3
 
 /* Bytes of device workspace cg_create needs for an n-row system: the vectors
- * r, p, p', q, z, D^-1 (each n doubles, 256-byte aligned), the per-CTA reduction
- * partials, the device-resident scalar state and the grid-barrier word. */
+ * r, p, q, D^-1 and one spare (each n doubles, 256-byte aligned), a padded copy of rowptr
+ * (n + 41 ints), the per-CTA reduction partials, the grid all-reduce inboxes (1.8 MB) and
+ * the device-resident scalar state. */
 size_t cg_workspace_bytes(int64_t n);
 
 /* Bind a handle to a CSR matrix already resident on the device.
  * d_rowptr int32[n+1], d_colind int32[nnz], d_vals double[nnz].
  * d_workspace: >= cg_workspace_bytes(n) bytes, 256-byte aligned.
- * Reads n+1 row pointers once (one stream-0 kernel) to pick the SpMV tiling.
+ * Reads the n+1 row pointers once (two stream-0 kernels: tile statistics, padded copy) to
+ * pick the SpMV variant and the ring geometry.
  * Errors: CG_EINVAL on NULL/misaligned pointers, n <= 0, nnz < 0, n or nnz
  * >= 2^31, workspace too small; CG_EUNSUPPORTED off sm_100; CG_ECUDA. */
 int cg_create(cg_handle** out, int64_t n, int64_t nnz,
@@ -114,18 +116,37 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
                   void* d_scratch, size_t scratch_bytes, void* cuda_stream);
 
 /* Tuning / diagnostics.  Options (name -> value):
- *   "loop"  0 = one cooperative persistent kernel (default)
- *           1 = CUDA graph of {K1, K2, K3} per iteration, replayed in chunks
- *               with a device-side stop flag (the profilable twin)
- *           2 = plain per-iteration launches, same kernels as 1
- *   "spmv"  0 = auto, 1 = sub-warp-per-row from global memory,
- *           2 = bulk-async (TMA) streamed tiles, thread per row
- *   "chunk" iterations per graph replay in loop mode 1 (even, default 32)
- * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches"
- * (kernels launched by the last call), "sms".
+ *   "loop"      0 = one cooperative persistent kernel (default)
+ *               1 = CUDA graph of {K1, K2, K3} per iteration, replayed in chunks
+ *                   with a device-side stop flag (the profilable twin)
+ *               2 = plain per-iteration launches, same kernels as 1
+ *   "spmv"      0 = auto; 1 = generic: sub-warp per row straight from global memory (any
+ *               CSR matrix); 2.. = streamed: warp-specialised bulk-async (TMA) producers,
+ *               a shared-memory ring of 32-row tiles and W consumer warps with one lane per
+ *               row and U entries in flight per lane: 2 = (W 12, U 9), 3 = (8, 27),
+ *               4 = (8, 9).  Falls back to 1 when a 32-row tile of the matrix does not fit
+ *               a ring of 8 slots (227 KB of shared memory).
+ *   "chunk"     iterations per graph replay in loop mode 1 (even, default 32)
+ *   "resident"  1 (default) = the persistent streamed kernel keeps x, r, p, q in registers
+ *               when every thread owns <= 4 rows; 0 = always in global memory
+ *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
+ *               started (default unlimited: the ring is refilled across the grid barriers)
+ *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant
+ * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
+ * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
+ * "consumer_warps", "in_flight", "ring_slots", "slot_bytes", "resident_rows".
  * Unknown names return CG_EINVAL. */
 int cg_set_option(cg_handle* h, const char* name, int64_t value);
 int cg_get_info(cg_handle* h, const char* name, int64_t* value);
+
+/* Read-bandwidth probe used by the bench for the L2 and HBM rooflines ("a
+ * read-only streaming microbenchmark over a 40 MB buffer, repeated, on the same box"): reads
+ * the `bytes` (>= 4096, 16-byte aligned) at d_buf `reps` times after one warm-up sweep, with
+ * 16-byte loads from every SM, and returns bytes * reps / time in *h_gbs (GB/s, CUDA events).
+ * A buffer smaller than the L2 measures L2 read bandwidth, a much larger one HBM read
+ * bandwidth.  Synchronises the stream. */
+int cg_probe_read_bandwidth(cg_handle* h, const void* d_buf, size_t bytes, int reps,
+                            double* h_gbs, void* cuda_stream);
 
 /* Phase trace of the persistent loop (loop mode 0), a profiling aid: with a non-NULL
  * d_trace (device uint64[grid * (iters + 1) * 16], grid = cg_get_info "grid"), thread 0 of every

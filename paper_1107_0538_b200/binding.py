@@ -33,6 +33,7 @@ SIGNATURES = {
                                        ctypes.POINTER(_f64), _vp]),
     "cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, _f64, _i64, _vp, ctypes.POINTER(_i64),
                                      ctypes.POINTER(_f64), _vp, _sz, _vp]),
+    "cg_probe_read_bandwidth": (ctypes.c_int, [_vp, _vp, _sz, ctypes.c_int, ctypes.POINTER(_f64), _vp]),
     "cg_set_trace": (ctypes.c_int, [_vp, _vp, _i64]),
     "cg_set_option": (ctypes.c_int, [_vp, ctypes.c_char_p, _i64]),
     "cg_get_info": (ctypes.c_int, [_vp, ctypes.c_char_p, ctypes.POINTER(_i64)]),
@@ -148,6 +149,14 @@ def cg_set_option(h: int, name: str, value: int) -> None:
         raise CGError(rc, f"cg_set_option({name}={value})")
 
 
+def cg_probe_read_bandwidth(h: int, d_buf: int, nbytes: int, reps: int, stream: int = 0) -> float:
+    out = _f64()
+    rc = lib().cg_probe_read_bandwidth(h, d_buf, nbytes, reps, ctypes.byref(out), stream)
+    if rc != 0:
+        raise CGError(rc, "cg_probe_read_bandwidth")
+    return out.value
+
+
 def cg_set_trace(h: int, d_trace: Optional[int], iters: int) -> None:
     rc = lib().cg_set_trace(h, d_trace, iters)
     if rc != 0:
@@ -220,6 +229,11 @@ class CG:
                                        device=self.device)
         cg_set_trace(self.h, self._trace.data_ptr(), iters)
         return self._trace
+
+    def probe_read_bandwidth(self, nbytes: int, reps: int = 20) -> float:
+        """GB/s of a read-only sweep over a scratch buffer of nbytes (L2 if it fits, else HBM)."""
+        buf = self.torch.ones(nbytes // 4, dtype=self.torch.int32, device=self.device)
+        return cg_probe_read_bandwidth(self.h, buf.data_ptr(), buf.numel() * 4, reps, self._stream())
 
     def check_csr(self) -> bool:
         return cg_check_csr(self.h, self._stream()) == 0

@@ -72,6 +72,20 @@ __global__ void __launch_bounds__(kThreads, 2) k_spmv(Params P, const double* x,
     phase_spmv_vector_dispatch<false>(P, x, y, blockIdx.x, gridDim.x);
 }
 
+// cg_probe_read_bandwidth: every thread streams 16-byte loads over the buffer.
+__global__ void __launch_bounds__(512) k_probe_read(const uint4* __restrict__ buf, size_t n16, unsigned* sink) {
+    unsigned acc = 0;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < n16; i += 4 * stride) {
+        const uint4 a = __ldcg(buf + i), b = __ldcg(buf + i + stride);
+        const uint4 c = __ldcg(buf + i + 2 * stride), d = __ldcg(buf + i + 3 * stride);
+        acc += a.x ^ b.y ^ c.z ^ d.w;
+    }
+    for (; i < n16; i += stride) acc += __ldcg(buf + i).x;
+    if (acc == 0x9e3779b9u) *sink = acc;              // never true for the buffers the bench passes: keeps the loads alive
+}
+
 // padded copy of rowptr for the streamed variants' 36-int bulk copies
 __global__ void k_pad_rowptr(const int* __restrict__ rowptr, long long n, int* __restrict__ out, long long total) {
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -331,7 +345,7 @@ struct cg_handle {
     Scal* h_scal; Params* h_params;        // pinned host mirrors
     int sms, smem_optin;
     size_t l2_bytes;
-    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead;
+    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots;
     int max_row_len, max_tile_nnz, tpr;
     bool dinv_ready;
     int grid_generic;                      // cooperative grid of the generic variant
@@ -378,8 +392,8 @@ static int setup_generic(cg_handle* h) {
     return CG_OK;
 }
 
-// Ring geometry from the matrix statistics, then per variant: does a ring of at least
-// W + 2 slots fit the opt-in shared memory?  (W slots may be held by consumers.)
+// Ring geometry from the matrix statistics; the streamed variants need a ring of at least
+// 2 * kProducers slots in the opt-in shared memory.
 static int setup_stream(cg_handle* h) {
     h->cap = (h->max_tile_nnz + 6 + 3) & ~3;
     if (h->cap < 4) h->cap = 4;
@@ -387,6 +401,7 @@ static int setup_stream(cg_handle* h) {
     const long long budget = (long long)h->smem_optin - cgs::kSmemTail;
     long long S = budget / h->slot_bytes;
     if (S > cgs::kMaxSlots) S = cgs::kMaxSlots;
+    if (S > h->max_slots) S = h->max_slots;
     // A slot must always be refilled by the same producer warp (tile j -> warp j mod kProducers,
     // slot j mod S): otherwise a warp could run two phases ahead of a slot's "empty" barrier,
     // which a parity wait cannot tell from zero phases ahead.
@@ -394,7 +409,7 @@ static int setup_stream(cg_handle* h) {
     h->slots = (int)S;
     for (int v = 0; v < kNumStream; ++v) {
         const StreamFns& f = stream_fns(v);
-        h->stream_ok[v] = S >= f.W + 2 && h->sms <= cgs::kBarGrid;
+        h->stream_ok[v] = S >= 2 * cgs::kProducers && h->sms <= cgs::kBarGrid;   // slots are released early: S need not cover W
         if (!h->stream_ok[v]) continue;
         const int smem = h->smem_optin;      // the attribute is per function, not per handle: always the maximum
         const void* fns[] = {f.spmv, f.init_spmv, f.init_residual, f.init_scalars, f.k1, f.k2, f.k3,
@@ -469,7 +484,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     h->sms = prop.multiProcessorCount;
     h->smem_optin = (int)prop.sharedMemPerBlockOptin;
     h->l2_bytes = (size_t)prop.l2CacheSize;
-    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30;
+    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_params, sizeof(Params), cudaHostAllocDefault);
@@ -528,6 +543,12 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!strcmp(name, "spmv")) { if (value < 0 || value > 1 + kNumStream) return CG_EINVAL; h->spmv_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "chunk")) { if (value < 2 || value > 4096 || (value & 1)) return CG_EINVAL; h->chunk = (int)value; return CG_OK; }
     if (!strcmp(name, "lookahead")) { if (value < 0 || value > (1 << 30)) return CG_EINVAL; h->lookahead = (int)value; return CG_OK; }
+    if (!strcmp(name, "ring_slots")) {
+        if (value < 2 * cgs::kProducers || value > cgs::kMaxSlots) return CG_EINVAL;
+        h->max_slots = (int)value;
+        if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // captured with the old smem size
+        return setup_stream(h);
+    }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "tpr")) {
         if (value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return CG_EINVAL;
@@ -579,6 +600,31 @@ extern "C" int cg_set_trace(cg_handle* h, uint64_t* d_trace, int64_t iters) {
         return CG_EINVAL;
     h->trace = (d_trace && iters > 0) ? reinterpret_cast<unsigned long long*>(d_trace) : nullptr;
     h->trace_iters = h->trace ? (int)iters : 0;
+    return CG_OK;
+}
+
+extern "C" int cg_probe_read_bandwidth(cg_handle* h, const void* d_buf, size_t bytes, int reps,
+                                       double* h_gbs, void* cuda_stream) {
+    if (!h || !d_buf || !h_gbs || bytes < 4096 || reps < 1 || !aligned16(d_buf)) return CG_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const size_t n16 = bytes / 16;
+    unsigned* sink = reinterpret_cast<unsigned*>(&h->scal->dot_out);
+    const uint4* buf = static_cast<const uint4*>(d_buf);
+    k_probe_read<<<h->sms * 4, 512, 0, st>>>(buf, n16, sink);          // warm-up (and L2 fill)
+    cudaEventRecord(e0, st);
+    for (int r = 0; r < reps; ++r) k_probe_read<<<h->sms * 4, 512, 0, st>>>(buf, n16, sink);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    CK(e);
+    CK(cudaGetLastError());
+    h->launches = reps + 1;
+    *h_gbs = (double)(n16 * 16) * reps / ((double)ms * 1e-3) / 1e9;
     return CG_OK;
 }
 

@@ -56,6 +56,7 @@ struct Ring {
     uint64_t* empty;
     double* red;                      // 104 doubles of reduction scratch (see kRedTot)
     volatile int* ctl;                // [0] stop flag, [1] passes consumed (low), [2] (high), [3] passes started
+    volatile unsigned* tag;           // per slot: 1 + number (mod 2^32) of the tile last issued into it
     int S, slot_bytes, cap;
     unsigned long long* acc;          // optional: cycles this thread waited on full barriers (trace)
     __device__ __forceinline__ double* vals(int slot) const {
@@ -78,6 +79,7 @@ __device__ __forceinline__ Ring ring_view(const Params& P, unsigned char* dyn) {
     rg.empty = rg.full + kMaxSlots;
     rg.red = reinterpret_cast<double*>(rg.empty + kMaxSlots);
     rg.ctl = reinterpret_cast<volatile int*>(rg.red + 104);
+    rg.tag = reinterpret_cast<volatile unsigned*>(rg.ctl + 8);
     return rg;
 }
 
@@ -86,6 +88,7 @@ __device__ __forceinline__ void ring_init(const Ring& rg) {
     if ((int)threadIdx.x < rg.S) {
         mbar_init(&rg.full[threadIdx.x], 1);
         mbar_init(&rg.empty[threadIdx.x], 1);
+        rg.tag[threadIdx.x] = 0u;
     }
     if (threadIdx.x == 0) { rg.ctl[0] = 0; rg.ctl[1] = 0; rg.ctl[2] = 0; rg.ctl[3] = 0; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -109,7 +112,7 @@ __device__ __forceinline__ void cta_tiles(const Params& P, int cta, int G, long 
 // ---------------------------------------------------------------- producer
 
 __device__ __forceinline__ void producer_issue(const Params& P, const Ring& rg, int slot, long long t,
-                                               int s, int e, uint64_t policy) {
+                                               int s, int e, uint64_t policy, unsigned tag) {
     const int s4 = s & ~3;
     const int lim = (int)(P.nnz & ~3LL);              // last entry reachable by bulk copies
     int e4 = (e + 3) & ~3;
@@ -124,6 +127,7 @@ __device__ __forceinline__ void producer_issue(const Params& P, const Ring& rg, 
         }
     }
     uint64_t* bar = &rg.full[slot];
+    rg.tag[slot] = tag;                               // before the arrive below (release): see consume_tile
     mbar_expect_tx(bar, (uint32_t)cnt * 12u + (uint32_t)kRpInts * 4u);
     if (cnt > 0) {
         if (P.l2_stream) {
@@ -139,11 +143,11 @@ __device__ __forceinline__ void producer_issue(const Params& P, const Ring& rg, 
 
 // A pass starts at ring position `pos` = (slot index, parity) of its tile 0; tile j of the pass
 // sits j slots further on.
-struct RingPos { unsigned slot; unsigned par; };
+struct RingPos { unsigned slot; unsigned par; unsigned seq; };      // seq: tile number mod 2^32
 __device__ __forceinline__ RingPos ring_advance(const Ring& rg, RingPos p, unsigned tiles) {
     const unsigned t = p.slot + tiles;
     const unsigned q = t / (unsigned)rg.S;
-    RingPos r; r.slot = t - q * (unsigned)rg.S; r.par = p.par ^ (q & 1u);
+    RingPos r; r.slot = t - q * (unsigned)rg.S; r.par = p.par ^ (q & 1u); r.seq = p.seq + tiles;
     return r;
 }
 
@@ -202,7 +206,7 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
             const int src = cached ? j : l;
             const int si = __shfl_sync(0xffffffffu, s, src);
             const int ei = __shfl_sync(0xffffffffu, e, src);
-            if (lane == 0) producer_issue(P, rg, (int)slot, tb + j, si, ei, policy);
+            if (lane == 0) producer_issue(P, rg, (int)slot, tb + j, si, ei, policy, (unsigned)seq + 1u);
             seq += (unsigned long long)NP;
             j += NP;
             while (j >= Tc) { j -= Tc; ++pass; }
@@ -254,6 +258,11 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
     static_assert(U % 3 == 0, "three accumulators");
     const RingPos at = ring_advance(rg, pos, (unsigned)j);
     const int slot = (int)at.slot;
+    // The parity wait below cannot tell "this tile has landed" from "the slot's PREVIOUS tile
+    // has not landed yet" (two phases apart).  The previous tile belongs to another warp, and
+    // bulk copies complete out of order, so first wait until this tile has been issued into
+    // the slot: from then on the barrier's pending phase is this tile's.
+    while (rg.tag[slot] != at.seq + 1u) { }
     if (rg.acc) {
         const long long t0 = clock64();
         mbar_wait(&rg.full[slot], at.par);

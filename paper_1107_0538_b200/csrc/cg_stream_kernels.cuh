@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_spmv(Params P, const
     CGS_PROLOGUE(W);
     ring_init(rg);
     if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
-    phase_spmv_tiles<W, U, false>(P, rg, x, y, tb, Tc, RingPos{0u, 0u});
+    phase_spmv_tiles<W, U, false>(P, rg, x, y, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
 // ---- stand-alone kernels of loop modes 1 (graph) and 2 (stepwise).  They read Params from
@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_spmv(const Para
     CGS_PROLOGUE(W);
     ring_init(rg);
     if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
-    phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, RingPos{0u, 0u});
+    phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
 template <int W>
@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks1_spmv_dot(const Para
     if (cta == 0 && threadIdx.x == 0) P.scal->brk[s] = 0;
     ring_init(rg);
     if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
-    const double d = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, RingPos{0u, 0u});
+    const double d = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, RingPos{0u, 0u, 0u});
     const double t = block_sum_w<W>(d, rg.red);
     if (threadIdx.x == 0) P.part0[cta] = t;
 }
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
     Scal* S = P.scal;
     unsigned bcount = 0;
     unsigned long long pass = 0;
-    RingPos pos{0u, 0u};
+    RingPos pos{0u, 0u, 0u};
     constexpr int RR = R > 0 ? R : 1;
     double xr[RR], rv[RR], pv[RR], qv[RR], dv[RR];
     long long row[RR];

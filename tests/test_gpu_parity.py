@@ -86,7 +86,7 @@ def check_solve_parity(res, x, ref, iters_band=True):
 # ---------------------------------------------------------------- SpMV / dot
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 def test_spmv_parity(bound, orc, cfg, variant):
     B = bound(cfg)
     p = B.p
@@ -172,7 +172,7 @@ def test_dot_parity(bound, orc, n):
 # ---------------------------------------------------------------- cg_solve
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 def test_solve_parity_persistent(bound, orc, cfg, variant):
     B = bound(cfg)
     p = B.p
@@ -213,6 +213,55 @@ def test_loop_modes_agree_bitwise(bound, cfg):
     B.cg.set_option("loop", 0)
     B.cg.set_option("spmv", 0)
     assert abs(outs[0][2] - outs[1][2]) <= 1           # the two SpMV variants differ only by rounding
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_streamed_persistent_modes_agree_bitwise(bound, cfg):
+    """The streamed persistent kernel with x, r, p, q in registers, the same kernel with the
+    vectors in global memory, with and without producer run-ahead across the grid barriers,
+    and the graph twin all perform the same operations in the same order: identical bits."""
+    B = bound(cfg)
+    p = B.p
+    for variant in (2, 3):
+        B.cg.set_option("spmv", variant)
+        runs = []
+        for loop, resident, lookahead in ((0, 1, 1 << 30), (0, 0, 1 << 30), (0, 1, 0), (0, 0, 3), (1, 1, 1 << 30)):
+            B.cg.set_option("loop", loop)
+            B.cg.set_option("resident", resident)
+            B.cg.set_option("lookahead", lookahead)
+            if loop == 0 and resident == 1 and cfg != 1:          # config 1 has 5-7 rows per thread: global vectors
+                assert B.cg.info("resident_rows") in (2, 4)
+            x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+            runs.append((x.cpu().numpy().copy(), res.hist.cpu().numpy().copy(), res.iters, res.status))
+        for other in runs[1:]:
+            assert other[2] == runs[0][2] and other[3] == runs[0][3]
+            assert np.array_equal(other[1], runs[0][1])
+            assert np.array_equal(other[0], runs[0][0])
+    for name, v in (("loop", 0), ("resident", 1), ("lookahead", 1 << 30), ("spmv", 0)):
+        B.cg.set_option(name, v)
+
+
+def test_phase_trace_and_bandwidth_probe(bound, cgmod):
+    """cg_set_trace fills monotone clock stamps for every CTA; cg_probe_read_bandwidth returns
+    a plausible figure (both are profiling aids of include/cg.h)."""
+    B = bound(2)
+    p = B.p
+    B.cg.set_option("loop", 0)
+    iters = 12
+    tr = B.cg.trace(iters)
+    st, it, res = cgmod.cg_solve(B.cg.h, B.b.data_ptr(), torch.zeros_like(B.b).data_ptr(), 0.0, iters, None,
+                                 torch.cuda.current_stream().cuda_stream)
+    assert it == iters and st == 1
+    t = tr.cpu().numpy()
+    assert t.shape == (B.cg.info("grid"), iters + 1, 16)
+    stamps = t[:, :iters - 1, :8]
+    assert (stamps > 0).all() and (np.diff(stamps, axis=2) > 0).all()
+    assert t[:, iters, 2].max() > 0                      # tiles issued by producer warp 0
+    B.cg.trace(0)
+    gbs = B.cg.probe_read_bandwidth(32 << 20, reps=10)
+    assert 500.0 < gbs < 50000.0
+    with pytest.raises(cgmod.CGError):
+        cgmod.cg_probe_read_bandwidth(B.cg.h, 0, 1 << 20, 1, 0)
 
 
 def test_graph_chunk_sizes_and_launch_count(bound):
