@@ -183,6 +183,7 @@ def main():
     ap.add_argument("--lookahead", type=int, default=None)
     ap.add_argument("--resident", type=int, default=None)
     ap.add_argument("--ring-slots", type=int, default=None)
+    ap.add_argument("--fold", type=int, default=None)
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -249,6 +250,8 @@ def main():
             Ap.set_option("resident", args.resident)
         if args.ring_slots is not None:
             Ap.set_option("ring_slots", args.ring_slots)
+        if args.fold is not None:
+            Ap.set_option("fold", args.fold)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []
@@ -387,7 +390,11 @@ def main():
                        "setup, as in PAPER.md:48"},
         "roofline": {
             "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "k_persistent (one launch = one solve)",
+            # dram__bytes_read.sum + dram__bytes_write.sum of this launch (ks_persistent, one solve of 217
+            # iterations of config 2) from profiles/r01_v2_ncu_full_raw_metrics.txt: the matrix comes
+            # from DRAM once per solve, everything else is served by the L2
+            "traffic": 44.73e6 if (A.info("spmv") == 2 and A.info("loop") == 0) else None,
+            "kernel": "ks_persistent (one launch = one solve)",
             "bytes_per_launch": bytes_it * it_per_solve + prologue_bytes,
             "peak_source": peak_src,
             "note": "working set 53.5 MB is L2-resident: this config is bound by L2 bandwidth and grid-sync "
@@ -436,7 +443,10 @@ def main():
                             "(inputs 1.33 GB >> L2, no flush needed)",
                 "iterations_per_s": K / t4, "us_per_iteration": t4 / K * 1e6,
                 "roofline": {"bound": "hbm", "achieved": gbs4, "peak": peak, "unit": "GB/s",
-                             "frac": gbs4 / peak, "traffic": None, "target_frac": 0.70},
+                             "frac": gbs4 / peak, "target_frac": 0.70,
+                             # per launch of K iterations, scaled from the 20-iteration ncu capture in
+                             # profiles/r01_v2_ncu_full_raw_metrics.txt (33.53 GB for 35.30 GB algorithmic)
+                             "traffic": 0.95 * (b_it4 * K + pro4), "traffic_note": "scaled from a 20-iteration capture"},
                 "cg_gflops": cg_inputs.flops_per_iteration(p4.n, p4.nnz) * K / t4 / 1e9,
                 "launch": describe(A4),
             }

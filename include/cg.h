@@ -129,6 +129,12 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *   "chunk"     iterations per graph replay in loop mode 1 (even, default 32)
  *   "resident"  1 (default) = the persistent streamed kernel keeps x, r, p, q in registers
  *               when every thread owns <= 4 rows; 0 = always in global memory
+ *   "fold"      persistent streamed kernel with vectors in registers, no preconditioner:
+ *               1 = fold K3 into the next K1 (every gathered p_j is recomputed on the fly as
+ *               fma(beta, p_old_j, r_j), the owner's own expression, so results keep their
+ *               bits) and synchronise the grid twice instead of three times per iteration;
+ *               0 = off; 2 (default) = on when a CTA has <= 8 tiles (K1 is short)
+ *   "ring_slots" cap on the ring depth (8..32, rounded down to a multiple of 4)
  *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
  *               started (default unlimited: the ring is refilled across the grid barriers)
  *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant

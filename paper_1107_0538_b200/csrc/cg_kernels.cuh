@@ -79,6 +79,8 @@ struct Params {
     int cap;              // entries per ring slot (multiple of 4)
     int slots;            // ring depth S
     int slot_bytes;       // cap * 12 + 144, rounded up to 128
+    double* p2;           // second p buffer of the folded loop (cg_stream_kernels.cuh)
+    int fold;             // 1: fold K3 into the next K1's gathers (two grid syncs per iteration)
     int lookahead;        // producer run-ahead (tiles) into a pass the consumers have not started
     int l2_stream;        // 1: the matrix does not fit the L2 -> evict-first hint on its copies
 };

@@ -252,9 +252,14 @@ __device__ __forceinline__ void consumers_stop(const Ring& rg, unsigned long lon
 // registers -- before the gathers, which are the long-latency part: with U >= the row
 // length a slot is held for a few hundred cycles only and nearly the whole ring is in
 // flight.  Padding entries (k >= ke) use value 0 and column 0.
-template <int U>
+//
+// FOLD: the gathered operand is not stored anywhere yet: it is p_new[c] = fma(beta, p_old[c],
+// r[c]), the very expression K3 evaluates for row c, recomputed here by every thread that
+// needs it (x = p_old, r = the residual K2 just stored).  Same operation, same operands, same
+// bits as the owner's own update; it saves the third grid synchronisation of an iteration.
+template <int U, bool FOLD = false>
 __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, RingPos pos, int j,
-                                               int lane) {
+                                               int lane, const double* r = nullptr, double beta = 0.0) {
     static_assert(U % 3 == 0, "three accumulators");
     const RingPos at = ring_advance(rg, pos, (unsigned)j);
     const int slot = (int)at.slot;
@@ -300,6 +305,13 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) xv[u] = ld_global_f64(x + c[u]);
+        if constexpr (FOLD) {
+            double rg_[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) rg_[u] = ld_global_f64(r + c[u]);
+#pragma unroll
+            for (int u = 0; u < U; ++u) xv[u] = fma(beta, xv[u], rg_[u]);
+        }
 #pragma unroll
         for (int u = 0; u < U; u += 3) {
             a0 = fma(v[u], xv[u], a0);

@@ -237,6 +237,12 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
         ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
     unsigned long long full_wait = 0;
     if (tr) rg.acc = &full_wait;
+    // Folded loop (R > 0, no preconditioner, option "fold"): two grid synchronisations per
+    // iteration.  cur = which p buffer holds the p the next plain gather / fold would read.
+    const bool fold = R > 0 && !PRE && P.fold != 0;
+    bool have_beta = false;
+    double beta_prev = 0.0;
+    int cur = 0;
 #define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
     while (!stop) {
         CGS_STAMP(k, 0);
@@ -244,12 +250,35 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
         double dot = 0.0;
         consumers_begin_pass(rg, pass);
         if constexpr (R > 0) {
+            const double* psrc = cur ? P.p2 : P.p;
+            if (fold && have_beta) {
+                // K3 folded in: p = r + beta p for the rows this thread owns (registers, and
+                // the other p buffer for next iteration's gathers) ...
+                double* pdst = cur ? P.p : P.p2;
 #pragma unroll
-            for (int kk = 0; kk < R; ++kk) {
-                const int j = warp + kk * W;
-                if (j < Tc) {
-                    qv[kk] = consume_tile<U>(rg, P.p, pos, j, lane);
-                    if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                for (int kk = 0; kk < R; ++kk) {
+                    if (row[kk] < 0) continue;
+                    pv[kk] = fma(beta_prev, pv[kk], rv[kk]);
+                    pdst[row[kk]] = pv[kk];
+                }
+                // ... and, recomputed on the fly, for every column the SpMV gathers
+#pragma unroll
+                for (int kk = 0; kk < R; ++kk) {
+                    const int j = warp + kk * W;
+                    if (j < Tc) {
+                        qv[kk] = consume_tile<U, true>(rg, psrc, pos, j, lane, P.r, beta_prev);
+                        if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                    }
+                }
+                cur ^= 1;
+            } else {
+#pragma unroll
+                for (int kk = 0; kk < R; ++kk) {
+                    const int j = warp + kk * W;
+                    if (j < Tc) {
+                        qv[kk] = consume_tile<U>(rg, psrc, pos, j, lane);
+                        if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                    }
                 }
             }
         } else {
@@ -275,6 +304,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
                 rv[kk] = fma(na, qv[kk], rv[kk]);
                 arr = fma(rv[kk], rv[kk], arr);
                 if (PRE) arz = fma(rv[kk], dv[kk] * rv[kk], arz);
+                if (fold) P.r[row[kk]] = rv[kk];          // gathered by the next K1
             }
         } else {
             phase_xr_tiles<W, PRE>(P, alpha, tb, Tc, arr, arz);
@@ -283,7 +313,8 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
         double v2[PRE ? 2 : 1];
         v2[0] = arr;
         if (PRE) v2[PRE ? 1 : 0] = arz;
-        grid_allreduce<W, (PRE ? 2 : 1), false>(P, rg.red, bcount, cta, G, v2);
+        if (fold) grid_allreduce<W, (PRE ? 2 : 1), true>(P, rg.red, bcount, cta, G, v2);      // publishes r and p
+        else      grid_allreduce<W, (PRE ? 2 : 1), false>(P, rg.red, bcount, cta, G, v2);
         CGS_STAMP(k, 4);
         // scalar beta, continue-condition
         const double rr_new = v2[0];
@@ -296,6 +327,12 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
         if (lead && P.hist) P.hist[k] = res;
         if (res <= thresh) { stop = 1; status = CG_OK; break; }
         if (k >= P.maxit) { stop = 1; status = CG_MAXIT; break; }
+        if (fold) {                        // K3 happens inside the next K1
+            have_beta = true; beta_prev = beta;
+            CGS_STAMP(k - 1, 6);
+            CGS_STAMP(k - 1, 7);
+            continue;
+        }
         // K3: p = r + beta p
         if constexpr (R > 0) {
 #pragma unroll

@@ -217,18 +217,22 @@ def test_loop_modes_agree_bitwise(bound, cfg):
 
 @pytest.mark.parametrize("cfg", [0, 1, 2])
 def test_streamed_persistent_modes_agree_bitwise(bound, cfg):
-    """The streamed persistent kernel with x, r, p, q in registers, the same kernel with the
-    vectors in global memory, with and without producer run-ahead across the grid barriers,
-    and the graph twin all perform the same operations in the same order: identical bits."""
+    """The streamed persistent kernel with x, r, p, q in registers (with K3 folded into the next
+    K1's gathers, two grid syncs per iteration, or not), the same kernel with the vectors in
+    global memory, with and without producer run-ahead across the grid barriers, and the graph
+    twin all perform the same operations in the same order: identical bits."""
     B = bound(cfg)
     p = B.p
     for variant in (2, 3):
         B.cg.set_option("spmv", variant)
         runs = []
-        for loop, resident, lookahead in ((0, 1, 1 << 30), (0, 0, 1 << 30), (0, 1, 0), (0, 0, 3), (1, 1, 1 << 30)):
+        big = 1 << 30
+        for loop, resident, lookahead, fold in ((0, 1, big, 1), (0, 1, big, 0), (0, 0, big, 1), (0, 1, 0, 1),
+                                                (0, 0, 3, 0), (1, 1, big, 1)):
             B.cg.set_option("loop", loop)
             B.cg.set_option("resident", resident)
             B.cg.set_option("lookahead", lookahead)
+            B.cg.set_option("fold", fold)
             if loop == 0 and resident == 1 and cfg != 1:          # config 1 has 5-7 rows per thread: global vectors
                 assert B.cg.info("resident_rows") in (2, 4)
             x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
@@ -237,7 +241,7 @@ def test_streamed_persistent_modes_agree_bitwise(bound, cfg):
             assert other[2] == runs[0][2] and other[3] == runs[0][3]
             assert np.array_equal(other[1], runs[0][1])
             assert np.array_equal(other[0], runs[0][0])
-    for name, v in (("loop", 0), ("resident", 1), ("lookahead", 1 << 30), ("spmv", 0)):
+    for name, v in (("loop", 0), ("resident", 1), ("lookahead", 1 << 30), ("fold", 1), ("spmv", 0)):
         B.cg.set_option(name, v)
 
 
