@@ -184,6 +184,7 @@ def main():
     ap.add_argument("--resident", type=int, default=None)
     ap.add_argument("--ring-slots", type=int, default=None)
     ap.add_argument("--fold", type=int, default=None)
+    ap.add_argument("--l2-hints", type=int, default=None)
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -252,6 +253,8 @@ def main():
             Ap.set_option("ring_slots", args.ring_slots)
         if args.fold is not None:
             Ap.set_option("fold", args.fold)
+        if args.l2_hints is not None:
+            Ap.set_option("l2_hints", args.l2_hints)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []

@@ -134,6 +134,8 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               fma(beta, p_old_j, r_j), the owner's own expression, so results keep their
  *               bits) and synchronise the grid twice instead of three times per iteration;
  *               0 = off; 2 (default) = on when a CTA has <= 8 tiles (K1 is short)
+ *   "l2_hints"  1 = evict_last / evict_first L2 hints on q between K1 and K2 when the matrix
+ *               exceeds the L2 (default 0: measured a net loss, see cg_stream.cuh)
  *   "ring_slots" cap on the ring depth (8..32, rounded down to a multiple of 4)
  *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
  *               started (default unlimited: the ring is refilled across the grid barriers)

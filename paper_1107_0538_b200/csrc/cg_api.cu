@@ -345,7 +345,7 @@ struct cg_handle {
     Scal* h_scal; Params* h_params;        // pinned host mirrors
     int sms, smem_optin;
     size_t l2_bytes;
-    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt;
+    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, l2_hints;
     int max_row_len, max_tile_nnz, tpr;
     bool dinv_ready;
     int grid_generic;                      // cooperative grid of the generic variant
@@ -448,7 +448,7 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     // irregular (config 3: 38 -> 60 us per iteration).  2 = auto.
     const long long tc_max = ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
     P->fold = h->fold_opt == 2 ? (tc_max <= 8 ? 1 : 0) : h->fold_opt;
-    P->l2_stream = ((size_t)h->nnz * 12u > h->l2_bytes / 2) ? 1 : 0;
+    P->l2_stream = ((size_t)h->nnz * 12u > h->l2_bytes / 2) ? (h->l2_hints ? 3 : 1) : 0;
 }
 
 extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
@@ -490,7 +490,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     h->sms = prop.multiProcessorCount;
     h->smem_optin = (int)prop.sharedMemPerBlockOptin;
     h->l2_bytes = (size_t)prop.l2CacheSize;
-    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2;
+    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->l2_hints = 0;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_params, sizeof(Params), cudaHostAllocDefault);
@@ -555,6 +555,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // captured with the old smem size
         return setup_stream(h);
     }
+    if (!strcmp(name, "l2_hints")) { if (value < 0 || value > 1) return CG_EINVAL; h->l2_hints = (int)value; return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "tpr")) {
@@ -576,7 +577,7 @@ static int resident_rows(const cg_handle* h, int v) {
     const long long tc_max = (ntiles + h->sms - 1) / h->sms;
     const int W = stream_fns(v - 2).W;
     const long long need = (tc_max + W - 1) / W;
-    return need <= 2 ? 2 : need <= 4 ? 4 : 0;
+    return need <= 2 ? 2 : need <= 4 ? 4 : 0;        // 8 rows per thread spill and gain nothing (measured on config 1)
 }
 
 extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {

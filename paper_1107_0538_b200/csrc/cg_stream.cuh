@@ -483,6 +483,25 @@ __device__ __forceinline__ void st_cs_f64(double* p, double v) {
     asm volatile("st.global.cs.f64 [%0], %1;" :: "l"(p), "d"(v) : "memory");
 }
 
+// Optional L2 residency hints for the big-system path (option "l2_hints", off by default).  q
+// is written by K1 and read by K2 a whole matrix sweep (1.3 GB at config 4) later: its stores
+// ask the L2 to keep the lines (evict_last), the one read in K2 releases them (evict_first).
+// Measured at config 4: K2 55.6 k instead of 59.9 k cycles, but K3 28.2 k instead of 16.2 k
+// (r and p lose their place in the L2): a net loss, hence off.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void st_hint_f64(double* p, double v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" :: "l"(p), "d"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ double ld_hint_f64(const double* p, uint64_t pol) {
+    double v;
+    asm volatile("ld.global.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+
 constexpr int kVU = 4;
 
 // Prologue: r = b - q (q = A x0); p = r (or D^-1 r); partials of r.r, b.b, r.z.
@@ -534,7 +553,8 @@ __device__ __forceinline__ void phase_xr_tiles(const Params& P, double alpha, lo
             idx[u] = (j < Tc && i < P.n) ? i : -1;
             if (idx[u] >= 0) {
                 xv[u] = ld_cs_f64(P.x + i); rv[u] = ld_global_f64(P.r + i);
-                pv[u] = ld_global_f64(P.p + i); qv[u] = ld_global_f64(P.q + i);
+                pv[u] = ld_global_f64(P.p + i);
+                qv[u] = P.l2_stream ? ld_hint_f64(P.q + i, l2_policy_evict_first()) : ld_global_f64(P.q + i);
                 if (PRE) dv[u] = P.dinv[i];
             }
         }
@@ -600,7 +620,8 @@ __device__ __forceinline__ double phase_spmv_tiles(const Params& P, const Ring& 
         if (DOT && row < P.n) xr = ld_global_f64(x + row);      // early: off the critical path
         const double acc = consume_tile<U>(rg, x, pos, j, lane);
         if (row < P.n) {
-            y[row] = acc;
+            if (P.l2_stream & 2) st_hint_f64(y + row, acc, l2_policy_evict_last());
+            else y[row] = acc;
             if (DOT) dot = fma(acc, xr, dot);
         }
     }
