@@ -168,6 +168,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
     const bool lead = cta == 0 && threadIdx.x == 0;
     Scal* S = P.scal;
     unsigned bcount = 0;
+    unsigned long long nbar = 0;
     unsigned long long pass = 0;
     RingPos pos{0u, 0u, 0u};
     constexpr int RR = R > 0 ? R : 1;
@@ -346,9 +347,8 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
             phase_p_tiles<W, PRE>(P, beta, tb, Tc);
         }
         CGS_STAMP(k - 1, 6);
-        double v0[1] = {0.0};
-        grid_allreduce<W, 1, true>(P, rg.red, bcount, cta, G, v0,       // publishes p
-                              (tr && k - 1 < P.trace_iters) ? tr + (k - 1) * kTraceSlots + 8 : nullptr);
+        grid_barrier_counter<W>(P, nbar, G,                               // publishes p
+                                (tr && k - 1 < P.trace_iters) ? tr + (k - 1) * kTraceSlots + 8 : nullptr);
         CGS_STAMP(k - 1, 7);
     }
 #undef CGS_STAMP
