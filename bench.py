@@ -101,6 +101,24 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def reduce_over_ranks(dist, value, op, device):
+    """MAX or SUM of one float over the ranks of the job (identity when dist is None).
+    Replicas only: the only cross-rank traffic of the bench is this bookkeeping."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def whole_job_value(dist, device, iterations_this_rank, seconds_this_rank):
+    """iterations of ALL ranks / MAX over ranks of the device time (weak scaling, replicas)."""
+    t = reduce_over_ranks(dist, seconds_this_rank, "max", device)
+    n = reduce_over_ranks(dist, iterations_this_rank, "sum", device)
+    return n / t, n, t
+
+
 def describe(A):
     """Launch configuration of a bound handle, from cg_get_info."""
     v = A.info("spmv")
@@ -212,18 +230,10 @@ def main():
         torch.cuda.synchronize()
 
     def max_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_over_ranks(dist, v, "max", "cuda")
 
     def sum_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return reduce_over_ranks(dist, v, "sum", "cuda")
 
     peak, peak_src = measured_peaks()
     dev = torch.device("cuda", local)
@@ -332,9 +342,7 @@ def main():
     barrier()
     t_wall1 = time.time()
     ms = [a.elapsed_time(b_) for a, b_ in ev]
-    t_dev = max_over_ranks(sum(ms) / 1e3)
-    iters_all = sum_over_ranks(iters_total)
-    value = iters_all / t_dev
+    value, iters_all, t_dev = whole_job_value(dist, "cuda", iters_total, sum(ms) / 1e3)
     clocks = sampler.stop(t_wall0, t_wall1)
     it_per_solve = iters_total / args.steps
     kernel_ms = float(np.mean(ms))

@@ -1,5 +1,5 @@
 // cg_stream.cuh -- the streamed CG path for sm_100a: warp-specialised bulk-async (TMA)
-// producer, W consumer warps with one lane per row, grid all-reduce fused with the grid
+// producers, W consumer warps with one lane per row, grid all-reduce fused with the grid
 // barrier, and (for systems small enough) x, r, p, q kept in registers for the whole solve.
 //
 // What is computed is unchanged ("DGEMV(sparse)" + the CG of
@@ -14,15 +14,16 @@
 // registers, persistent with vectors in global memory, graph, stepwise) performs the same
 // floating-point operations in the same order and gives bitwise identical results.
 //
-// K1 data flow.  One extra warp (the producer) walks the CTA's tiles in order and, for each,
-// waits for a free ring slot and issues three cp.async.bulk copies (SASS UBLKCP) into it:
-// the tile's contiguous vals span, its colind span and its 33 row pointers (36 ints from a
-// padded copy of rowptr).  Consumers wait on the slot's "full" mbarrier, read their row
-// bounds and entries from shared memory, gather x through L1/L2, and release the slot.  No
-// consumer ever waits on a row-pointer or matrix load from global memory; the only global
-// loads in its loop are the x gathers.  In the persistent kernel the producer runs ahead
-// into the next iteration's tiles (the matrix does not change) while the consumers do
-// K2/K3 and wait at the grid barriers, so K1 starts on a full ring.
+// K1 data flow.  kProducers extra warps (the producers) walk the CTA's tiles in order and,
+// for each, wait for a free ring slot and issue three cp.async.bulk copies (SASS UBLKCP)
+// into it: the tile's contiguous vals span, its colind span and its 33 row pointers (36
+// ints from a padded copy of rowptr).  Consumers wait on the slot's "full" mbarrier, copy
+// their row bounds and entries from shared memory into registers, hand the slot back, then
+// gather x through L1/L2.  No consumer ever waits on a row-pointer or matrix load from
+// global memory; the only global loads in its loop are the x gathers.  In the persistent
+// kernel the producers run ahead into the next iteration's tiles (the matrix does not
+// change) while the consumers do K2/K3 and wait at the grid barriers, so K1 starts on a
+// full ring.
 //
 // Alignment of the bulk copies: source, destination and size must be multiples of 16
 // bytes.  A tile's span [s, e) is widened to [s & ~3, (e + 3) & ~3), clamped to nnz & ~3;

@@ -191,6 +191,50 @@ def test_solve_parity_persistent(bound, orc, cfg, variant):
     B.cg.set_option("spmv", 0)
 
 
+def _banded_spd(n, half_band):
+    """SPD band matrix with 2*half_band + 1 entries per interior row (longer than the 27 the
+    streamed consumer handles in one trip): off-diagonals -1/(d+1), strictly dominant diagonal."""
+    rows, cols, vals = [], [], []
+    for i in range(n):
+        lo, hi = max(0, i - half_band), min(n - 1, i + half_band)
+        js = np.arange(lo, hi + 1)
+        v = -1.0 / (np.abs(js - i) + 1.0)
+        v[js == i] = 0.0
+        v[js == i] = np.abs(v).sum() + 0.05
+        rows.append(len(js)); cols.append(js); vals.append(v)
+    rp = np.zeros(n + 1, dtype=np.int32)
+    np.cumsum(rows, out=rp[1:])
+    return rp, np.concatenate(cols).astype(np.int32), np.concatenate(vals)
+
+
+@pytest.mark.parametrize("half_band", [30, 36, 45])
+def test_solve_long_rows_streamed(cgmod, orc, half_band):
+    """Rows of 61 / 73 / 91 entries: several trips per row in the streamed consumer, few ring slots
+    (a tile is 2-3 times a 27-point one), and past that the fall-back to the generic path; all
+    variants and loop modes against the oracle."""
+    n = 5003
+    rp, ci, va = _banded_spd(n, half_band)
+    b = gi.seeded_vector(77, n)
+    ref = orc.cg(rp, ci, va, b, rtol=1e-10, maxit=n)
+    cg = cgmod.CG(dev(rp), dev(ci), dev(va))
+    assert cg.info("stream_ok") == (1 if half_band <= 36 else 0)
+    outs = []
+    for variant in (2, 3, 4):
+        cg.set_option("spmv", variant)
+        if half_band > 36:               # a 32-row tile no longer fits a ring of 8 slots: generic path
+            assert cg.info("spmv") == 1
+        else:
+            assert cg.info("spmv") == variant and cg.info("ring_slots") >= 8
+        for loop in (0, 1):
+            cg.set_option("loop", loop)
+            x, res = cg.solve(dev(b), rtol=1e-10, maxit=n)
+            check_solve_parity(res, x, ref)
+            outs.append((variant, x.cpu().numpy().copy()))
+    for (va_, xa), (vb_, xb) in zip(outs[::2], outs[1::2]):
+        assert va_ == vb_ and np.array_equal(xa, xb)             # persistent == graph twin, per variant
+    cg.close()
+
+
 @pytest.mark.parametrize("cfg", [0, 2])
 def test_loop_modes_agree_bitwise(bound, cfg):
     """Persistent kernel, CUDA-graph replay and plain launches share the phase code and the
