@@ -1,4 +1,8 @@
-// cg_kernels.cuh -- device code of the fp64 CSR conjugate-gradient hot path for sm_100a.
+// cg_kernels.cuh -- shared device code of the fp64 CSR conjugate-gradient hot path for sm_100a:
+// the parameter / state structs, load-store and mbarrier / bulk-copy primitives, and the
+// GENERIC variant ("spmv" = 1): sub-warp per row straight from global memory, grid-stride
+// vector phases, a counter grid barrier.  The default, streamed variant lives in
+// cg_stream.cuh / cg_stream_kernels.cuh.
 //
 // Steps (the paper names only the first, PAPER.md:44
 // "Tasks, such as DGEMV(sparse), are repetitive"; the rest is the textbook CG of
@@ -11,9 +15,9 @@
 // in a fixed order -- the paper's CPU-side scalar step and its transfers
 // do not exist here.
 //
-// The same phase functions are used by the persistent cooperative kernel and by
-// the three stand-alone kernels of the graph / stepwise loop, so all loop modes
-// give bitwise identical results for equal grid and block sizes.
+// Within a variant the same phase functions are used by the persistent cooperative kernel
+// and by the three stand-alone kernels of the graph / stepwise loop, so all loop modes give
+// bitwise identical results.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
