@@ -136,6 +136,8 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               0 = off; 2 (default) = on when a CTA has <= 8 tiles (K1 is short)
  *   "l2_hints"  1 = evict_last / evict_first L2 hints on q between K1 and K2 when the matrix
  *               exceeds the L2 (default 0: measured a net loss, see cg_stream.cuh)
+ *   "l2_prefetch" n > 0: producers prefetch n of their tiles (1 = 8) into the L2 ahead of the
+ *               ring copies when the matrix exceeds the L2 (default 0: measured no gain)
  *   "ring_slots" cap on the ring depth (8..32, rounded down to a multiple of 4)
  *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
  *               started (default unlimited: the ring is refilled across the grid barriers)

@@ -345,7 +345,7 @@ struct cg_handle {
     Scal* h_scal; Params* h_params;        // pinned host mirrors
     int sms, smem_optin;
     size_t l2_bytes;
-    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, l2_hints;
+    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, l2_hints, l2_prefetch;
     int max_row_len, max_tile_nnz, tpr;
     bool dinv_ready;
     int grid_generic;                      // cooperative grid of the generic variant
@@ -442,6 +442,7 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     P->rp_pad = h->rp_pad; P->bslots = h->bslots;
     P->cap = h->cap; P->slots = h->slots; P->slot_bytes = h->slot_bytes;
     P->lookahead = h->lookahead;
+    P->l2_prefetch = h->l2_prefetch;
     P->p2 = h->spare;
     // Folding K3 into the next K1 trades a grid synchronisation for a second gather per entry:
     // measured a gain only while K1 is short (<= 8 tiles per CTA), a loss when gathers are
@@ -490,7 +491,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     h->sms = prop.multiProcessorCount;
     h->smem_optin = (int)prop.sharedMemPerBlockOptin;
     h->l2_bytes = (size_t)prop.l2CacheSize;
-    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->l2_hints = 0;
+    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->l2_hints = 0; h->l2_prefetch = 0;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_params, sizeof(Params), cudaHostAllocDefault);
@@ -555,6 +556,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // captured with the old smem size
         return setup_stream(h);
     }
+    if (!strcmp(name, "l2_prefetch")) { if (value < 0 || value > 32) return CG_EINVAL; h->l2_prefetch = (int)value; return CG_OK; }
     if (!strcmp(name, "l2_hints")) { if (value < 0 || value > 1) return CG_EINVAL; h->l2_hints = (int)value; return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }

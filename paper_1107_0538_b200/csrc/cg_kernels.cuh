@@ -86,6 +86,7 @@ struct Params {
     double* p2;           // second p buffer of the folded loop (cg_stream_kernels.cuh)
     int fold;             // 1: fold K3 into the next K1's gathers (two grid syncs per iteration)
     int lookahead;        // producer run-ahead (tiles) into a pass the consumers have not started
+    int l2_prefetch;      // 1: producers prefetch tiles into the L2 a batch ahead (only with l2_stream)
     int l2_stream;        // 1: the matrix does not fit the L2 -> evict-first hint on its copies
 };
 

@@ -142,6 +142,24 @@ __device__ __forceinline__ void producer_issue(const Params& P, const Ring& rg, 
     bulk_g2s_plain(rg.rp(slot), P.rp_pad + t * kTileRows, (uint32_t)kRpInts * 4u, bar);
 }
 
+constexpr int kPrefetchBatch = 8;    // tiles per producer warp sent towards the L2 ahead of their ring copies
+
+// Start a tile's vals / colind spans towards the L2 (same widening and clamping as producer_issue).
+__device__ __forceinline__ void prefetch_tile_l2(const Params& P, int s, int e) {
+    const int s4 = s & ~3;
+    const int lim = (int)(P.nnz & ~3LL);
+    int e4 = (e + 3) & ~3;
+    if (e4 > lim) e4 = lim;
+    const int cnt = e4 > s4 ? e4 - s4 : 0;
+    if (cnt > 0) {
+        const uint64_t pol = l2_policy_evict_first();      // must not push p out of the L2
+        asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;"
+                     :: "l"(P.vals + s4), "r"((uint32_t)cnt * 8u), "l"(pol) : "memory");
+        asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;"
+                     :: "l"(P.colind + s4), "r"((uint32_t)cnt * 4u), "l"(pol) : "memory");
+    }
+}
+
 // A pass starts at ring position `pos` = (slot index, parity) of its tile 0; tile j of the pass
 // sits j slots further on.
 struct RingPos { unsigned slot; unsigned par; unsigned seq; };      // seq: tile number mod 2^32
@@ -180,17 +198,35 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
         s = ld_stream_s32(P.rp_pad + (tb + lane) * kTileRows);
         e = ld_stream_s32(P.rp_pad + (tb + lane) * kTileRows + kTileRows);
     }
+    // Optional (option "l2_prefetch", off by default), matrix >> L2: the producers start every
+    // tile towards the L2 one batch of their tiles before they copy it into shared memory
+    // (cp.async.bulk.prefetch.L2 needs no slot and no barrier), to have more bytes in flight
+    // towards HBM than the ring holds.  Measured at config 4: with 4 tiles per warp ahead K1
+    // drops from 451 k to 429 k cycles on average but the CTAs drift apart (the barrier
+    // after K1 grows from 16 k to 40 k cycles): no gain; 8 and 16 ahead are slower outright.
+    const bool pf = P.l2_stream != 0 && P.l2_prefetch != 0;
+    const int B = cached ? 32 : (pf ? (P.l2_prefetch > 1 ? P.l2_prefetch : kPrefetchBatch) : 32);
+    if (!cached && lane < B) {             // bounds of my first batch
+        const int jl = (int)(((long long)j + (long long)lane * NP) % Tc);
+        s = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows);
+        e = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows + kTileRows);
+        if (pf) prefetch_tile_l2(P, s, e);
+    }
     bool stopped = false;
     unsigned long long t_wait = 0;
     const long long t_begin = clock64();
     const bool timing = P.trace != nullptr;
     while (pass < passes && !stopped) {
-        if (!cached) {                     // bounds of my next 32 tiles
-            const int jl = (int)(((long long)j + (long long)lane * NP) % Tc);
-            s = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows);
-            e = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows + kTileRows);
+        int s2 = 0, e2 = 0;
+        if (!cached) {                     // bounds of the batch AFTER this one; start them towards the L2
+            const int jl = (int)(((long long)j + (long long)(B + lane) * NP) % Tc);
+            if (lane < B) {
+                s2 = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows);
+                e2 = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows + kTileRows);
+                if (pf) prefetch_tile_l2(P, s2, e2);
+            }
         }
-        for (int l = 0; l < 32 && pass < passes; ++l) {
+        for (int l = 0; l < B && pass < passes; ++l) {
             int ok = 1;
             if (lane == 0) {
                 const long long t0 = timing ? clock64() : 0;
@@ -214,6 +250,7 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
             slot += (unsigned)NP;
             if (slot >= (unsigned)rg.S) { slot -= (unsigned)rg.S; par ^= 1u; }
         }
+        if (!cached) { s = s2; e = e2; }
     }
     if (timing && lane == 0 && q == 0) {   // producer statistics in the row after the last traced iteration
         unsigned long long* row = P.trace + ((size_t)blockIdx.x * (P.trace_iters + 1) + P.trace_iters) * kTraceSlots;
