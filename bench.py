@@ -204,6 +204,7 @@ def main():
     ap.add_argument("--fold", type=int, default=None)
     ap.add_argument("--l2-hints", type=int, default=None)
     ap.add_argument("--l2-prefetch", type=int, default=None)
+    ap.add_argument("--pin", type=int, default=None)
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -268,6 +269,8 @@ def main():
             Ap.set_option("l2_hints", args.l2_hints)
         if args.l2_prefetch is not None:
             Ap.set_option("l2_prefetch", args.l2_prefetch)
+        if args.pin is not None:
+            Ap.set_option("pin", args.pin)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []

@@ -138,7 +138,10 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               exceeds the L2 (default 0: measured a net loss, see cg_stream.cuh)
  *   "l2_prefetch" n > 0: producers prefetch n of their tiles (1 = 8) into the L2 ahead of the
  *               ring copies when the matrix exceeds the L2 (default 0: measured no gain)
- *   "ring_slots" cap on the ring depth (8..32, rounded down to a multiple of 4)
+ *   "pin"       1 (default) = when every CTA's slice of the matrix fits its ring (up to 64
+ *               tiles in 225 KB of shared memory per SM), copy it there once per solve and
+ *               keep it; 0 = stream everything every iteration
+ *   "ring_slots" cap on the ring depth (8..64, rounded down to a multiple of 4)
  *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
  *               started (default unlimited: the ring is refilled across the grid barriers)
  *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant

@@ -345,7 +345,7 @@ struct cg_handle {
     Scal* h_scal; Params* h_params;        // pinned host mirrors
     int sms, smem_optin;
     size_t l2_bytes;
-    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, l2_hints, l2_prefetch;
+    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, l2_hints, l2_prefetch, pin_opt;
     int max_row_len, max_tile_nnz, tpr;
     bool dinv_ready;
     int grid_generic;                      // cooperative grid of the generic variant
@@ -450,6 +450,18 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     const long long tc_max = ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
     P->fold = h->fold_opt == 2 ? (tc_max <= 8 ? 1 : 0) : h->fold_opt;
     P->l2_stream = ((size_t)h->nnz * 12u > h->l2_bytes / 2) ? (h->l2_hints ? 3 : 1) : 0;
+    // Pinned tiles (cg_stream.cuh): when every CTA's slice of the matrix fits the ring, it is
+    // copied into shared memory once per solve and stays there.
+    P->pinned = 0; P->stream_slots = h->slots;
+    if (h->pin_opt && !P->l2_stream && variant >= 2) {
+        if (tc_max <= h->slots) {
+            P->pinned = (int)tc_max;
+            P->stream_slots = (h->slots - (int)tc_max) / cgs::kProducers * cgs::kProducers;
+        }
+        // A partial split (pin S - 8 tiles, stream the rest through 8 slots) was measured on
+        // config 2 and lost: K1 12.4 k against 10.2 k cycles, the streamed tiles queue up
+        // behind too few slots.  The kernels support it; the host never asks for it.
+    }
 }
 
 extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
@@ -491,7 +503,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     h->sms = prop.multiProcessorCount;
     h->smem_optin = (int)prop.sharedMemPerBlockOptin;
     h->l2_bytes = (size_t)prop.l2CacheSize;
-    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->l2_hints = 0; h->l2_prefetch = 0;
+    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->l2_hints = 0; h->l2_prefetch = 0; h->pin_opt = 1;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_params, sizeof(Params), cudaHostAllocDefault);
@@ -555,6 +567,12 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         h->max_slots = (int)value;
         if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // captured with the old smem size
         return setup_stream(h);
+    }
+    if (!strcmp(name, "pin")) {
+        if (value < 0 || value > 1) return CG_EINVAL;
+        h->pin_opt = (int)value;
+        if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // kernels read it from Params, but be safe
+        return CG_OK;
     }
     if (!strcmp(name, "l2_prefetch")) { if (value < 0 || value > 32) return CG_EINVAL; h->l2_prefetch = (int)value; return CG_OK; }
     if (!strcmp(name, "l2_hints")) { if (value < 0 || value > 1) return CG_EINVAL; h->l2_hints = (int)value; return CG_OK; }

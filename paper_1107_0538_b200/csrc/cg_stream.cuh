@@ -40,8 +40,8 @@ constexpr int kRpPad = 40;           // extra ints at the end of the padded rowp
 constexpr int kBarVals = 3;          // values per grid all-reduce
 constexpr int kBarGrid = 160;        // max CTAs of a streamed persistent grid (1 per SM; B200 has 148)
 constexpr int kBarM = kBarGrid / 32;
-constexpr int kMaxSlots = 32;
-constexpr int kSmemTail = 1536;      // mbarriers + reduction scratch + flags after the slots
+constexpr int kMaxSlots = 64;
+constexpr int kSmemTail = 2304;      // mbarriers + reduction scratch + flags after the slots
 constexpr int kRedTot = 96;          // red[0..95]: per-warp partials (3 values x 32 warps); red[96..]: totals
 
 constexpr int kProducers = 4;        // producer warps per CTA (W + kProducers is a multiple of 4)
@@ -59,6 +59,7 @@ struct Ring {
     volatile int* ctl;                // [0] stop flag, [1] passes consumed (low), [2] (high), [3] passes started
     volatile unsigned* tag;           // per slot: 1 + number (mod 2^32) of the tile last issued into it
     int S, slot_bytes, cap;
+    int P, Q;                         // pinned slots [0, P) and streaming slots [P, P + Q), P + Q <= S
     unsigned long long* acc;          // optional: cycles this thread waited on full barriers (trace)
     __device__ __forceinline__ double* vals(int slot) const {
         return reinterpret_cast<double*>(slots + (size_t)slot * slot_bytes);
@@ -74,13 +75,14 @@ struct Ring {
 __device__ __forceinline__ Ring ring_view(const Params& P, unsigned char* dyn) {
     Ring rg;
     rg.S = P.slots; rg.slot_bytes = P.slot_bytes; rg.cap = P.cap; rg.acc = nullptr;
+    rg.P = P.pinned; rg.Q = P.stream_slots;
     rg.slots = dyn;
     unsigned char* tail = dyn + (size_t)P.slots * P.slot_bytes;
     rg.full = reinterpret_cast<uint64_t*>(tail);
     rg.empty = rg.full + kMaxSlots;
     rg.red = reinterpret_cast<double*>(rg.empty + kMaxSlots);
     rg.ctl = reinterpret_cast<volatile int*>(rg.red + 104);
-    rg.tag = reinterpret_cast<volatile unsigned*>(rg.ctl + 8);
+    rg.tag = reinterpret_cast<volatile unsigned*>(rg.ctl + 8);       // kMaxSlots entries
     return rg;
 }
 
@@ -160,14 +162,27 @@ __device__ __forceinline__ void prefetch_tile_l2(const Params& P, int s, int e) 
     }
 }
 
-// A pass starts at ring position `pos` = (slot index, parity) of its tile 0; tile j of the pass
-// sits j slots further on.
-struct RingPos { unsigned slot; unsigned par; unsigned seq; };      // seq: tile number mod 2^32
+// Pinned and streamed tiles.  When the matrix is L2-resident anyway (it is re-read every
+// iteration), the first P tiles of a CTA are PINNED: tile j < P is copied into slot j once,
+// in the first pass, and stays there for the whole solve (no L2 traffic, no shared-memory
+// write, no producer work for it in later iterations).  The other Ts = Tc - P tiles of a
+// pass are STREAMED through the Q slots [P, P + Q): streamed tile number seq (counted over
+// all passes) uses slot P + seq mod Q.  P = Tc (everything pinned, nothing streamed) when
+// the CTA's whole slice fits the ring.
+//
+// A pass starts at stream position `pos` = (slot offset, parity, number) of its first streamed
+// tile; streamed tile i of the pass sits i slots further on.
+struct RingPos { unsigned slot; unsigned par; unsigned seq; };      // seq: streamed tile number mod 2^32
 __device__ __forceinline__ RingPos ring_advance(const Ring& rg, RingPos p, unsigned tiles) {
+    const unsigned Q = rg.Q > 0 ? (unsigned)rg.Q : 1u;
     const unsigned t = p.slot + tiles;
-    const unsigned q = t / (unsigned)rg.S;
-    RingPos r; r.slot = t - q * (unsigned)rg.S; r.par = p.par ^ (q & 1u); r.seq = p.seq + tiles;
+    const unsigned q = t / Q;
+    RingPos r; r.slot = t - q * Q; r.par = p.par ^ (q & 1u); r.seq = p.seq + tiles;
     return r;
+}
+// Position of the next pass: a pass streams Tc - P tiles.
+__device__ __forceinline__ RingPos ring_next_pass(const Ring& rg, RingPos p, int Tc) {
+    return Tc > rg.P ? ring_advance(rg, p, (unsigned)(Tc - rg.P)) : p;
 }
 
 // Producer warp q of NP.  The CTA's tiles form one endless sequence: `passes` sweeps over
@@ -187,17 +202,38 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     const int lane = threadIdx.x & 31;
     const uint64_t policy = l2_policy_evict_first();
     if (Tc <= 0) return;
-    unsigned long long seq = (unsigned long long)q;        // next tile number I issue
-    long long pass = 0;
-    int j = q;                                              // = seq - pass * Tc
-    while (j >= Tc) { j -= Tc; ++pass; }
-    unsigned slot = (unsigned)q, par = 0;                   // = seq mod S, (seq / S) & 1
+    const int Pn = rg.P < Tc ? rg.P : Tc;                  // my CTA's pinned tiles: [0, Pn)
+    const int Ts = Tc - Pn;                                 // streamed tiles per pass
+    const int Q = rg.Q;
     int s = 0, e = 0;
-    const bool cached = Tc <= 32;
+    const bool cached = Tc <= 32;                           // lane l keeps the bounds of tile l
     if (cached && lane < Tc) {
         s = ld_stream_s32(P.rp_pad + (tb + lane) * kTileRows);
         e = ld_stream_s32(P.rp_pad + (tb + lane) * kTileRows + kTileRows);
     }
+    // Pinned tiles: mine are j = q, q + NP, ... < Pn; each goes into slot j once (its slot was
+    // never used: no empty wait).  Lane l fetches the bounds of my l-th one (Pn <= 64).
+    {
+        int ps = 0, pe = 0;
+        const int mine = Pn > q ? (Pn - q + NP - 1) / NP : 0;
+        if (!cached && lane < mine) {
+            const long long t = tb + q + (long long)lane * NP;
+            ps = ld_stream_s32(P.rp_pad + t * kTileRows);
+            pe = ld_stream_s32(P.rp_pad + t * kTileRows + kTileRows);
+        }
+        for (int l = 0; l < mine; ++l) {
+            const int j = q + l * NP;
+            const int si = __shfl_sync(0xffffffffu, cached ? s : ps, cached ? j : l);
+            const int ei = __shfl_sync(0xffffffffu, cached ? e : pe, cached ? j : l);
+            if (lane == 0) producer_issue(P, rg, j, tb + j, si, ei, policy, (unsigned)j + 1u);
+        }
+    }
+    if (Ts <= 0 || Q <= 0) return;
+    unsigned long long seq = (unsigned long long)q;        // next streamed tile number I issue
+    long long pass = 0;
+    int j = q;                                              // = seq - pass * Ts, index among the streamed tiles
+    while (j >= Ts) { j -= Ts; ++pass; }
+    unsigned slot = (unsigned)q, par = 0;                   // = seq mod Q, (seq / Q) & 1
     // Optional (option "l2_prefetch", off by default), matrix >> L2: the producers start every
     // tile towards the L2 one batch of their tiles before they copy it into shared memory
     // (cp.async.bulk.prefetch.L2 needs no slot and no barrier), to have more bytes in flight
@@ -207,9 +243,9 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     const bool pf = P.l2_stream != 0 && P.l2_prefetch != 0;
     const int B = cached ? 32 : (pf ? (P.l2_prefetch > 1 ? P.l2_prefetch : kPrefetchBatch) : 32);
     if (!cached && lane < B) {             // bounds of my first batch
-        const int jl = (int)(((long long)j + (long long)lane * NP) % Tc);
-        s = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows);
-        e = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows + kTileRows);
+        const int jl = (int)(((long long)j + (long long)lane * NP) % Ts);
+        s = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows);
+        e = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows + kTileRows);
         if (pf) prefetch_tile_l2(P, s, e);
     }
     bool stopped = false;
@@ -219,10 +255,10 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     while (pass < passes && !stopped) {
         int s2 = 0, e2 = 0;
         if (!cached) {                     // bounds of the batch AFTER this one; start them towards the L2
-            const int jl = (int)(((long long)j + (long long)(B + lane) * NP) % Tc);
+            const int jl = (int)(((long long)j + (long long)(B + lane) * NP) % Ts);
             if (lane < B) {
-                s2 = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows);
-                e2 = ld_stream_s32(P.rp_pad + (tb + jl) * kTileRows + kTileRows);
+                s2 = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows);
+                e2 = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows + kTileRows);
                 if (pf) prefetch_tile_l2(P, s2, e2);
             }
         }
@@ -233,22 +269,22 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
                 if (passes > 1 && j >= P.lookahead) {
                     while ((long long)rg.ctl[3] <= pass) { if (rg.ctl[0]) { ok = 0; break; } }
                 }
-                while (ok && !mbar_try_wait(&rg.empty[slot], par ^ 1u)) {
+                while (ok && !mbar_try_wait(&rg.empty[Pn + slot], par ^ 1u)) {
                     if (rg.ctl[0]) ok = 0;
                 }
                 if (timing) t_wait += (unsigned long long)(clock64() - t0);
             }
             ok = __shfl_sync(0xffffffffu, ok, 0);
             if (!ok) { stopped = true; break; }
-            const int src = cached ? j : l;
+            const int src = cached ? Pn + j : l;
             const int si = __shfl_sync(0xffffffffu, s, src);
             const int ei = __shfl_sync(0xffffffffu, e, src);
-            if (lane == 0) producer_issue(P, rg, (int)slot, tb + j, si, ei, policy, (unsigned)seq + 1u);
+            if (lane == 0) producer_issue(P, rg, Pn + (int)slot, tb + Pn + j, si, ei, policy, (unsigned)seq + 1u);
             seq += (unsigned long long)NP;
             j += NP;
-            while (j >= Tc) { j -= Tc; ++pass; }
+            while (j >= Ts) { j -= Ts; ++pass; }
             slot += (unsigned)NP;
-            if (slot >= (unsigned)rg.S) { slot -= (unsigned)rg.S; par ^= 1u; }
+            if (slot >= (unsigned)Q) { slot -= (unsigned)Q; par ^= 1u; }
         }
         if (!cached) { s = s2; e = e2; }
     }
@@ -258,13 +294,13 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     }
     if (stopped) {
         // Drain: my copies for tiles nobody will consume must land before the CTA exits.  The
-        // consumers finished `done` whole passes, i.e. the tiles below done * Tc.
+        // consumers finished `done` whole passes, i.e. the streamed tiles below done * Ts.
         const unsigned long long done = (((unsigned long long)(unsigned)rg.ctl[2] << 32) | (unsigned)rg.ctl[1])
-                                        * (unsigned long long)Tc;
+                                        * (unsigned long long)Ts;
         unsigned long long w = done + (((unsigned long long)q + (unsigned long long)NP
                                         - done % (unsigned long long)NP) % (unsigned long long)NP);
         for (; w < seq; w += (unsigned long long)NP)
-            mbar_wait(&rg.full[(int)(w % (unsigned)rg.S)], (uint32_t)((w / (unsigned)rg.S) & 1ULL));
+            mbar_wait(&rg.full[Pn + (int)(w % (unsigned)Q)], (uint32_t)((w / (unsigned)Q) & 1ULL));
     }
 }
 
@@ -299,7 +335,10 @@ template <int U, bool FOLD = false>
 __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, RingPos pos, int j,
                                                int lane, const double* r = nullptr, double beta = 0.0) {
     static_assert(U % 3 == 0, "three accumulators");
-    const RingPos at = ring_advance(rg, pos, (unsigned)j);
+    const bool pinned = j < rg.P;
+    RingPos at;
+    if (pinned) { at.slot = (unsigned)j; at.par = 0u; at.seq = (unsigned)j; }        // its only phase
+    else { at = ring_advance(rg, pos, (unsigned)(j - rg.P)); at.slot += (unsigned)rg.P; }
     const int slot = (int)at.slot;
     // The parity wait below cannot tell "this tile has landed" from "the slot's PREVIOUS tile
     // has not landed yet" (two phases apart).  The previous tile belongs to another warp, and
@@ -320,7 +359,7 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
     const int* sc = rg.cols(slot);
     const int trips = __reduce_max_sync(0xffffffffu, (ke - ks + U - 1) / U);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-    if (trips == 0) {
+    if (trips == 0 && !pinned) {
         __syncwarp();
         if (lane == 0) mbar_arrive(&rg.empty[slot]);
     }
@@ -337,7 +376,7 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
             c[u] = ok ? cc : 0;
             v[u] = ok ? vv : 0.0;
         }
-        if (t == trips - 1) {
+        if (t == trips - 1 && !pinned) {
             __syncwarp();                  // every lane has its last entries in registers
             if (lane == 0) mbar_arrive(&rg.empty[slot]);
         }

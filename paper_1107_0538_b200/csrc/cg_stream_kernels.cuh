@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
         phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, pos);
         phase_init_tiles<W, PRE>(P, tb, Tc, arr, abb, arz);     // reads only this thread's own q
     }
-    ++pass; pos = ring_advance(rg, pos, (unsigned)Tc);
+    ++pass; pos = ring_next_pass(rg, pos, Tc);
     double rr, bb, rz;
     {
         double v[PRE ? 3 : 2];
@@ -285,7 +285,7 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P)
         } else {
             dot = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, pos);
         }
-        ++pass; pos = ring_advance(rg, pos, (unsigned)Tc);
+        ++pass; pos = ring_next_pass(rg, pos, Tc);
         CGS_STAMP(k, 1);
         double v1[1] = {dot};
         grid_allreduce<W, 1, false>(P, rg.red, bcount, cta, G, v1);

@@ -263,7 +263,8 @@ def test_loop_modes_agree_bitwise(bound, cfg):
 def test_streamed_persistent_modes_agree_bitwise(bound, cfg):
     """The streamed persistent kernel with x, r, p, q in registers (with K3 folded into the next
     K1's gathers, two grid syncs per iteration, or not), the same kernel with the vectors in
-    global memory, with and without producer run-ahead across the grid barriers, and the graph
+    global memory, with and without producer run-ahead across the grid barriers, with part of
+    the matrix pinned in shared memory or all of it streamed every iteration, and the graph
     twin all perform the same operations in the same order: identical bits."""
     B = bound(cfg)
     p = B.p
@@ -271,8 +272,10 @@ def test_streamed_persistent_modes_agree_bitwise(bound, cfg):
         B.cg.set_option("spmv", variant)
         runs = []
         big = 1 << 30
-        for loop, resident, lookahead, fold in ((0, 1, big, 1), (0, 1, big, 0), (0, 0, big, 1), (0, 1, 0, 1),
-                                                (0, 0, 3, 0), (1, 1, big, 1)):
+        for loop, resident, lookahead, fold, pin in ((0, 1, big, 1, 1), (0, 1, big, 0, 1), (0, 0, big, 1, 1),
+                                                     (0, 1, 0, 1, 1), (0, 0, 3, 0, 0), (1, 1, big, 1, 1),
+                                                     (0, 1, big, 0, 0), (1, 1, big, 1, 0)):
+            B.cg.set_option("pin", pin)
             B.cg.set_option("loop", loop)
             B.cg.set_option("resident", resident)
             B.cg.set_option("lookahead", lookahead)
@@ -285,7 +288,7 @@ def test_streamed_persistent_modes_agree_bitwise(bound, cfg):
             assert other[2] == runs[0][2] and other[3] == runs[0][3]
             assert np.array_equal(other[1], runs[0][1])
             assert np.array_equal(other[0], runs[0][0])
-    for name, v in (("loop", 0), ("resident", 1), ("lookahead", 1 << 30), ("fold", 1), ("spmv", 0)):
+    for name, v in (("loop", 0), ("resident", 1), ("lookahead", 1 << 30), ("fold", 2), ("pin", 1), ("spmv", 0)):
         B.cg.set_option(name, v)
 
 
