@@ -155,6 +155,31 @@ def time_oracle(problem, seconds_budget, fixed_iters=None):
     return total_it / dt, solves, total_it, dt
 
 
+def time_oracle_omp(problem, seconds_budget):
+    """oracle/cg_oracle_omp.c (row-parallel OpenMP build of the oracle's loops; checked against
+    the oracle in tests/test_oracle_pins.py) on all host cores and on half of them (containers
+    often expose more CPUs than they may use); the faster of the two is reported."""
+    from oracle import cg_oracle as orc
+    p = problem
+    ncpu = os.cpu_count() or 1
+    best = None
+    for threads in sorted({ncpu, max(1, ncpu // 2)}, reverse=True):
+        orc.omp_set_threads(threads)
+        orc.cg_omp(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)       # warm-up
+        its, solves, t0 = 0, 0, time.perf_counter()
+        while True:
+            its += orc.cg_omp(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit).iters
+            solves += 1
+            dt = time.perf_counter() - t0
+            if dt >= seconds_budget / 2:
+                break
+        rec = {"value": its / dt, "unit": UNIT, "cores": threads, "kind": "oracle loops + OpenMP (cg_oracle_omp.c)",
+               "sample": f"{solves} full solves of config{WORKLOAD_CFG} ({its} iterations, {dt:.1f} s)"}
+        if best is None or rec["value"] > best["value"]:
+            best = rec
+    return best
+
+
 def run_reference(args):
     """--impl reference: this tier's reference arm is the CPU oracle (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -477,6 +502,10 @@ def main():
         v, solves, its, dt = time_oracle(p, seconds_budget=10.0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"{solves} full solves of config{WORKLOAD_CFG} ({its} iterations, {dt:.1f} s)"}
+        try:        # the same loops with OpenMP on the host's cores, beside the oracle
+            line["cpu_allcores"] = time_oracle_omp(p, seconds_budget=4.0)
+        except Exception as e:
+            line["cpu_allcores"] = {"error": repr(e)}
     elif rank == 0:
         line["cpu_baseline"] = None
 

@@ -30,7 +30,21 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+_SRC_OMP = os.path.join(_HERE, "cg_oracle_omp.c")
+_LIB_OMP = os.path.join(_HERE, "libcg_oracle_omp.so")
+
+
+def build_omp(force: bool = False) -> str:
+    """Compile cg_oracle_omp.c (the all-cores baseline; not the parity reference)."""
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC_OMP):
+        tmp = _LIB_OMP + f".{os.getpid()}.tmp"
+        subprocess.check_call(["gcc", *_CFLAGS, "-fopenmp", "-o", tmp, _SRC_OMP, "-lm"])
+        os.replace(tmp, _LIB_OMP)
+    return _LIB_OMP
+
+
 _lib = None
+_lib_omp = None
 _c_i32p = ctypes.POINTER(ctypes.c_int32)
 _c_f64p = ctypes.POINTER(ctypes.c_double)
 
@@ -163,3 +177,47 @@ def cg(rowptr, colind, vals, b, x0=None, rtol=1e-10, maxit=None, dinv=None,
                     hist=hist[:k + 1].copy(), alpha=alpha[:k].copy(), beta=beta[:k].copy(),
                     P=None if P is None else P[:kk], R=None if R is None else R[:kk],
                     X=None if X is None else X[:kk])
+
+
+def omp_threads() -> int:
+    """Threads the OpenMP baseline uses (OMP_NUM_THREADS or all cores)."""
+    global _lib_omp
+    if _lib_omp is None:
+        _lib_omp = ctypes.CDLL(build_omp())
+    _lib_omp.oracle_omp_threads.restype = ctypes.c_int
+    return int(_lib_omp.oracle_omp_threads())
+
+
+def omp_set_threads(t: int) -> None:
+    global _lib_omp
+    if _lib_omp is None:
+        _lib_omp = ctypes.CDLL(build_omp())
+    _lib_omp.oracle_omp_set_threads.argtypes = [ctypes.c_int]
+    _lib_omp.oracle_omp_set_threads(int(t))
+
+
+def cg_omp(rowptr, colind, vals, b, x0=None, rtol=1e-10, maxit=None) -> CGResult:
+    """The same CG with row-parallel OpenMP loops on all host cores (cg_oracle_omp.c): the
+    all-cores CPU baseline of SURVEY.md 8(d), itself checked against `cg` in the tests."""
+    global _lib_omp
+    if _lib_omp is None:
+        _lib_omp = ctypes.CDLL(build_omp())
+    keepalive, args, n = _csr(rowptr, colind, vals)
+    if maxit is None:
+        maxit = n
+    bb, pb = _f64(b)
+    x = np.zeros(n, dtype=np.float64) if x0 is None else np.array(x0, dtype=np.float64, copy=True)
+    hist = np.zeros(maxit + 1, dtype=np.float64)
+    iters = ctypes.c_int64(0)
+    res = ctypes.c_double(0.0)
+    fn = _lib_omp.oracle_cg_omp
+    fn.argtypes = [ctypes.c_int64, _c_i32p, _c_i32p, _c_f64p, _c_f64p, _c_f64p, ctypes.c_double,
+                   ctypes.c_int64, _c_f64p, ctypes.POINTER(ctypes.c_int64), _c_f64p]
+    fn.restype = ctypes.c_int
+    st = fn(*args, pb, x.ctypes.data_as(_c_f64p), ctypes.c_double(rtol), ctypes.c_int64(maxit),
+            hist.ctypes.data_as(_c_f64p), ctypes.byref(iters), ctypes.byref(res))
+    if st < 0:
+        raise ValueError("oracle_cg_omp: invalid argument")
+    k = int(iters.value)
+    return CGResult(x=x, iters=k, status=int(st), resnorm=float(res.value), hist=hist[:k + 1].copy(),
+                    alpha=np.zeros(0), beta=np.zeros(0))

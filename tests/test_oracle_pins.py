@@ -323,3 +323,18 @@ def test_iteration_counts_reported_not_pinned(problems):
         p = problems(cfg)
         r = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
         assert r.status == 0 and lo <= r.iters <= hi, (cfg, r.iters)
+
+
+def test_openmp_baseline_matches_the_oracle(problems):
+    """cg_oracle_omp.c (all-cores CPU baseline of SURVEY.md 8(d)) is the same algorithm with
+    parallel loops: it must meet the tolerances the GPU path has to meet against the oracle."""
+    for cfg in (0, 2):
+        p = problems(cfg)
+        ref = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+        orc.omp_set_threads(2)
+        got = orc.cg_omp(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+        k = min(50, ref.iters)
+        assert np.max(np.abs(got.hist[:k + 1] - ref.hist[:k + 1]) / ref.hist[:k + 1]) <= 1e-9
+        assert abs(got.iters - ref.iters) <= max(1, int(0.02 * ref.iters))
+        assert np.linalg.norm(got.x - ref.x) / np.linalg.norm(ref.x) <= 1e-8
+        assert got.status == ref.status == 0
