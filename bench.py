@@ -127,7 +127,7 @@ def describe(A):
     if v == 1:
         d["spmv"] = f"generic: {A.info('tpr')} lanes per row from global memory"
     else:
-        d["spmv"] = (f"streamed: 4 TMA producer warps + {A.info('consumer_warps')} consumer warps, one lane per row, "
+        d["spmv"] = (f"streamed: {A.info('producer_warps')} TMA producer warps + {A.info('consumer_warps')} consumer warps, one lane per row, "
                      f"{A.info('in_flight')} gathers in flight per lane, ring of {A.info('ring_slots')} x "
                      f"{A.info('slot_bytes')} B tiles")
         rr = A.info("resident_rows")

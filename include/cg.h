@@ -123,8 +123,9 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *   "spmv"      0 = auto; 1 = generic: sub-warp per row straight from global memory (any
  *               CSR matrix); 2.. = streamed: warp-specialised bulk-async (TMA) producers,
  *               a shared-memory ring of 32-row tiles and W consumer warps with one lane per
- *               row and U entries in flight per lane: 2 = (W 12, U 9), 3 = (8, 27),
- *               4 = (8, 9).  Falls back to 1 when a 32-row tile of the matrix does not fit
+ *               row and U entries in flight per lane: 2 = (W 12, 4 producers, U 9),
+ *               3 = (8, 4, 27), 4 = (8, 4, 9), 5 = (11, 5, 9).  Auto picks 5 when the matrix is
+ *               re-streamed from the L2 every iteration, else 2.  Falls back to 1 when a 32-row tile of the matrix does not fit
  *               a ring of 8 slots (227 KB of shared memory).
  *   "chunk"     iterations per graph replay in loop mode 1 (even, default 32)
  *   "resident"  1 (default) = the persistent streamed kernel keeps x, r, p, q in registers
@@ -147,7 +148,7 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
- * "consumer_warps", "in_flight", "ring_slots", "slot_bytes", "resident_rows".
+ * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "slot_bytes", "resident_rows".
  * Unknown names return CG_EINVAL. */
 int cg_set_option(cg_handle* h, const char* name, int64_t value);
 int cg_get_info(cg_handle* h, const char* name, int64_t* value);

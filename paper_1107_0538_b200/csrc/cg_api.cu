@@ -300,38 +300,38 @@ static thread_local char g_cuda_err[256] = "no CUDA error recorded";
     } while (0)
 
 // Streamed variants: W consumer warps, U entries in flight per lane (cg_stream.cuh).
-// "spmv" option value = index + 2.  W + kProducers is a multiple of 4 so the warps spread evenly
-// over the SM's four sub-partitions (their register files bound the registers per thread).
+// "spmv" option value = index + 2.
 struct StreamFns {
-    int W, U;
+    int W, NP, U;
     const void* spmv;
     const void* init_spmv; const void* init_residual; const void* init_scalars;
     const void* k1; const void* k2; const void* k3;
     const void* persistent[3][2];          // [R index: 0 -> global vectors, 1 -> R = 2, 2 -> R = 4][Jacobi]
 };
 
-template <int W, int U> static StreamFns make_stream_fns() {
+template <int W, int NP, int U> static StreamFns make_stream_fns() {
     StreamFns f;
-    f.W = W; f.U = U;
-    f.spmv = (const void*)cgs::ks_spmv<W, U>;
-    f.init_spmv = (const void*)cgs::ks_init_spmv<W, U>;
-    f.init_residual = (const void*)cgs::ks_init_residual<W>;
-    f.init_scalars = (const void*)cgs::ks_init_scalars<W>;
-    f.k1 = (const void*)cgs::ks1_spmv_dot<W, U>;
-    f.k2 = (const void*)cgs::ks2_update_xr<W>;
-    f.k3 = (const void*)cgs::ks3_update_p<W>;
-    f.persistent[0][0] = (const void*)cgs::ks_persistent<W, U, 0, false>;
-    f.persistent[0][1] = (const void*)cgs::ks_persistent<W, U, 0, true>;
-    f.persistent[1][0] = (const void*)cgs::ks_persistent<W, U, 2, false>;
-    f.persistent[1][1] = (const void*)cgs::ks_persistent<W, U, 2, true>;
-    f.persistent[2][0] = (const void*)cgs::ks_persistent<W, U, 4, false>;
-    f.persistent[2][1] = (const void*)cgs::ks_persistent<W, U, 4, true>;
+    f.W = W; f.NP = NP; f.U = U;
+    f.spmv = (const void*)cgs::ks_spmv<W, NP, U>;
+    f.init_spmv = (const void*)cgs::ks_init_spmv<W, NP, U>;
+    f.init_residual = (const void*)cgs::ks_init_residual<W, NP>;
+    f.init_scalars = (const void*)cgs::ks_init_scalars<W, NP>;
+    f.k1 = (const void*)cgs::ks1_spmv_dot<W, NP, U>;
+    f.k2 = (const void*)cgs::ks2_update_xr<W, NP>;
+    f.k3 = (const void*)cgs::ks3_update_p<W, NP>;
+    f.persistent[0][0] = (const void*)cgs::ks_persistent<W, NP, U, 0, false>;
+    f.persistent[0][1] = (const void*)cgs::ks_persistent<W, NP, U, 0, true>;
+    f.persistent[1][0] = (const void*)cgs::ks_persistent<W, NP, U, 2, false>;
+    f.persistent[1][1] = (const void*)cgs::ks_persistent<W, NP, U, 2, true>;
+    f.persistent[2][0] = (const void*)cgs::ks_persistent<W, NP, U, 4, false>;
+    f.persistent[2][1] = (const void*)cgs::ks_persistent<W, NP, U, 4, true>;
     return f;
 }
-static constexpr int kNumStream = 3;
+static constexpr int kNumStream = 4;
 static const StreamFns& stream_fns(int idx) {
     static const StreamFns table[kNumStream] = {
-        make_stream_fns<12, 9>(), make_stream_fns<8, 27>(), make_stream_fns<8, 9>()};
+        make_stream_fns<12, 4, 9>(), make_stream_fns<8, 4, 27>(), make_stream_fns<8, 4, 9>(),
+        make_stream_fns<11, 5, 9>()};
     return table[idx];
 }
 
@@ -393,7 +393,7 @@ static int setup_generic(cg_handle* h) {
 }
 
 // Ring geometry from the matrix statistics; the streamed variants need a ring of at least
-// 2 * kProducers slots in the opt-in shared memory.
+// 8 slots in the opt-in shared memory, in a number the variant's producer count divides.
 static int setup_stream(cg_handle* h) {
     h->cap = (h->max_tile_nnz + 6 + 3) & ~3;
     if (h->cap < 4) h->cap = 4;
@@ -402,14 +402,15 @@ static int setup_stream(cg_handle* h) {
     long long S = budget / h->slot_bytes;
     if (S > cgs::kMaxSlots) S = cgs::kMaxSlots;
     if (S > h->max_slots) S = h->max_slots;
-    // A slot must always be refilled by the same producer warp (tile j -> warp j mod kProducers,
-    // slot j mod S): otherwise a warp could run two phases ahead of a slot's "empty" barrier,
-    // which a parity wait cannot tell from zero phases ahead.
-    S -= S % cgs::kProducers;
+    // A slot must always be refilled by the same producer warp (tile j -> warp j mod NP, slot
+    // j mod S): otherwise a warp could run two phases ahead of a slot's "empty" barrier, which
+    // a parity wait cannot tell from zero phases ahead.  So NP must divide S: multiples of 20
+    // serve both producer counts (4 and 5), shallower rings only the variants with 4.
+    S -= S % (S >= cgs::kSlotQuantum ? cgs::kSlotQuantum : 4);
     h->slots = (int)S;
     for (int v = 0; v < kNumStream; ++v) {
         const StreamFns& f = stream_fns(v);
-        h->stream_ok[v] = S >= 2 * cgs::kProducers && h->sms <= cgs::kBarGrid;   // slots are released early: S need not cover W
+        h->stream_ok[v] = S >= 8 && S % f.NP == 0 && h->sms <= cgs::kBarGrid;   // slots are released early: S need not cover W
         if (!h->stream_ok[v]) continue;
         const int smem = h->smem_optin;      // the attribute is per function, not per handle: always the maximum
         const void* fns[] = {f.spmv, f.init_spmv, f.init_residual, f.init_scalars, f.k1, f.k2, f.k3,
@@ -421,10 +422,18 @@ static int setup_stream(cg_handle* h) {
     return CG_OK;
 }
 
-// 1 = generic; 2 + i = streamed variant i.
+// 1 = generic; 2 + i = streamed variant i.  Auto: 12 consumer + 4 producer warps when the matrix
+// streams from HBM (config 4) or is pinned in shared memory (configs 0, 1: the producers
+// idle); 11 + 5 when it is re-streamed from the L2 every iteration (configs 2, 3: measured
+// 13.40 -> 12.68 and 34.28 -> 34.13 us per iteration; 292 -> 295 at config 4, 16.4 -> 17.2 at
+// config 1).
 static int pick_variant(const cg_handle* h) {
     if (h->spmv_opt == 1) return 1;
     if (h->spmv_opt >= 2) return h->stream_ok[h->spmv_opt - 2] ? h->spmv_opt : 1;
+    const long long tc_max = ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
+    const bool from_hbm = (size_t)h->nnz * 12u > h->l2_bytes / 2;
+    const bool pinned = h->pin_opt && !from_hbm && tc_max <= h->slots;
+    if (!from_hbm && !pinned && h->stream_ok[3]) return 5;
     return h->stream_ok[0] ? 2 : 1;
 }
 
@@ -456,7 +465,7 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     if (h->pin_opt && !P->l2_stream && variant >= 2) {
         if (tc_max <= h->slots) {
             P->pinned = (int)tc_max;
-            P->stream_slots = (h->slots - (int)tc_max) / cgs::kProducers * cgs::kProducers;
+            P->stream_slots = (h->slots - (int)tc_max) / cgs::kSlotQuantum * cgs::kSlotQuantum;   // unused: nothing streams
         }
         // A partial split (pin S - 8 tiles, stream the rest through 8 slots) was measured on
         // config 2 and lost: K1 12.4 k against 10.2 k cycles, the streamed tiles queue up
@@ -563,7 +572,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!strcmp(name, "chunk")) { if (value < 2 || value > 4096 || (value & 1)) return CG_EINVAL; h->chunk = (int)value; return CG_OK; }
     if (!strcmp(name, "lookahead")) { if (value < 0 || value > (1 << 30)) return CG_EINVAL; h->lookahead = (int)value; return CG_OK; }
     if (!strcmp(name, "ring_slots")) {
-        if (value < 2 * cgs::kProducers || value > cgs::kMaxSlots) return CG_EINVAL;
+        if (value < 8 || value > cgs::kMaxSlots) return CG_EINVAL;
         h->max_slots = (int)value;
         if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // captured with the old smem size
         return setup_stream(h);
@@ -606,7 +615,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     if (!strcmp(name, "loop")) *value = h->loop;
     else if (!strcmp(name, "spmv")) *value = v;
     else if (!strcmp(name, "grid")) *value = variant_grid(h, v);
-    else if (!strcmp(name, "block")) *value = v == 1 ? kThreads : 32 * (stream_fns(v - 2).W + cgs::kProducers);
+    else if (!strcmp(name, "block")) *value = v == 1 ? kThreads : 32 * (stream_fns(v - 2).W + stream_fns(v - 2).NP);
     else if (!strcmp(name, "smem")) *value = (int64_t)(v >= 2 ? stream_smem(h) : 0);
     else if (!strcmp(name, "launches")) *value = h->launches;
     else if (!strcmp(name, "sms")) *value = h->sms;
@@ -615,6 +624,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "max_tile_nnz")) *value = h->max_tile_nnz;
     else if (!strcmp(name, "stream_ok")) *value = h->stream_ok[0] ? 1 : 0;
     else if (!strcmp(name, "consumer_warps")) *value = v >= 2 ? stream_fns(v - 2).W : 0;
+    else if (!strcmp(name, "producer_warps")) *value = v >= 2 ? stream_fns(v - 2).NP : 0;
     else if (!strcmp(name, "in_flight")) *value = v >= 2 ? stream_fns(v - 2).U : 4;
     else if (!strcmp(name, "ring_slots")) *value = v >= 2 ? h->slots : 0;
     else if (!strcmp(name, "slot_bytes")) *value = v >= 2 ? h->slot_bytes : 0;
@@ -679,7 +689,7 @@ extern "C" int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_
     } else {
         const StreamFns& f = stream_fns(v - 2);
         void* args[] = {&P, &d_x, &d_y};
-        CK(cudaLaunchKernel(f.spmv, dim3(h->sms), dim3(32 * (f.W + cgs::kProducers)), args, stream_smem(h), st));
+        CK(cudaLaunchKernel(f.spmv, dim3(h->sms), dim3(32 * (f.W + f.NP)), args, stream_smem(h), st));
     }
     CK(cudaGetLastError());
     h->launches = 1;
@@ -714,7 +724,7 @@ static int launch_iteration_kernels(cg_handle* h, int v, cudaStream_t st, int it
             k3_update_p<<<G, kThreads, 0, st>>>(h->dparams, s);
         } else {
             const StreamFns& f = stream_fns(v - 2);
-            const dim3 blk(32 * (f.W + cgs::kProducers));
+            const dim3 blk(32 * (f.W + f.NP));
             const size_t smem = stream_smem(h);
             void* args[] = {&h->dparams, &s};
             CK(cudaLaunchKernel(f.k1, dim3(G), blk, args, smem, st));
@@ -772,7 +782,7 @@ static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, doubl
             const int ri = R == 2 ? 1 : R == 4 ? 2 : 0;
             h->last_resident = R;
             CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));        // arm the all-reduce slots
-            CK(cudaLaunchCooperativeKernel(f.persistent[ri][precond ? 1 : 0], dim3(G), dim3(32 * (f.W + cgs::kProducers)),
+            CK(cudaLaunchCooperativeKernel(f.persistent[ri][precond ? 1 : 0], dim3(G), dim3(32 * (f.W + f.NP)),
                                            args, stream_smem(h), st));
         }
         h->launches += 1;
@@ -785,7 +795,7 @@ static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, doubl
             k_init_scalars<<<G, kThreads, 0, st>>>(h->dparams);
         } else {
             const StreamFns& f = stream_fns(v - 2);
-            const dim3 blk(32 * (f.W + cgs::kProducers));
+            const dim3 blk(32 * (f.W + f.NP));
             const size_t smem = stream_smem(h);
             void* args[] = {&h->dparams};
             CK(cudaLaunchKernel(f.init_spmv, dim3(G), blk, args, smem, st));

@@ -83,7 +83,7 @@ struct Params {
     int cap;              // entries per ring slot (multiple of 4)
     int slots;            // ring depth S
     int pinned;           // P: tiles per CTA that stay in their slot for the whole solve
-    int stream_slots;     // Q: slots the other tiles stream through (multiple of kProducers)
+    int stream_slots;     // Q: slots the other tiles stream through (a multiple of the producer count)
     int slot_bytes;       // cap * 12 + 144, rounded up to 128
     double* p2;           // second p buffer of the folded loop (cg_stream_kernels.cuh)
     int fold;             // 1: fold K3 into the next K1's gathers (two grid syncs per iteration)

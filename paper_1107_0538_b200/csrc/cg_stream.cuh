@@ -14,7 +14,7 @@
 // registers, persistent with vectors in global memory, graph, stepwise) performs the same
 // floating-point operations in the same order and gives bitwise identical results.
 //
-// K1 data flow.  kProducers extra warps (the producers) walk the CTA's tiles in order and,
+// K1 data flow.  NP extra warps (the producers) walk the CTA's tiles in order and,
 // for each, wait for a free ring slot and issue three cp.async.bulk copies (SASS UBLKCP)
 // into it: the tile's contiguous vals span, its colind span and its 33 row pointers (36
 // ints from a padded copy of rowptr).  Consumers wait on the slot's "full" mbarrier, copy
@@ -44,12 +44,15 @@ constexpr int kMaxSlots = 64;
 constexpr int kSmemTail = 2304;      // mbarriers + reduction scratch + flags after the slots
 constexpr int kRedTot = 96;          // red[0..95]: per-warp partials (3 values x 32 warps); red[96..]: totals
 
-constexpr int kProducers = 4;        // producer warps per CTA (W + kProducers is a multiple of 4)
-template <int W> struct Shape {
+// W consumer warps + NP producer warps per CTA; W + NP is a multiple of 4 so the warps spread
+// evenly over the SM's four sub-partitions (their register files bound the registers per thread).
+template <int W, int NP> struct Shape {
     static constexpr int kConsumers = W;
+    static constexpr int kProducers = NP;
     static constexpr int kConsumerThreads = 32 * W;
-    static constexpr int kThreads = 32 * (W + kProducers);
+    static constexpr int kThreads = 32 * (W + NP);
 };
+constexpr int kSlotQuantum = 20;     // ring depths are multiples of this (lcm of the producer counts 4 and 5) when they can be
 
 struct Ring {
     unsigned char* slots;

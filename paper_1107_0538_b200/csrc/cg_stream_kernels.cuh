@@ -1,5 +1,5 @@
 // cg_stream_kernels.cuh -- kernel entry points of the streamed CG path (see cg_stream.cuh).
-// Every kernel is launched with 32 (W + kProducers) threads: W consumer warps and the producer
+// Every kernel is launched with 32 (W + NP) threads: W consumer warps and the producer
 // warps, which return at once in kernels that do not stream the matrix.
 #pragma once
 #include "cg_stream.cuh"
@@ -29,28 +29,28 @@ __device__ __forceinline__ void decide_start(const Params& P, double rr, double 
     (void)warp
 
 // ---- cg_spmv: y = A x
-template <int W, int U>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_spmv(Params P, const double* x, double* y) {
+template <int W, int NP, int U>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_spmv(Params P, const double* x, double* y) {
     CGS_PROLOGUE(W);
     ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, NP); return; }
     phase_spmv_tiles<W, U, false>(P, rg, x, y, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
 // ---- stand-alone kernels of loop modes 1 (graph) and 2 (stepwise).  They read Params from
 // ---- device memory so that a captured graph survives across solves.
 
-template <int W, int U>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_spmv(const Params* __restrict__ dp) {
+template <int W, int NP, int U>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_init_spmv(const Params* __restrict__ dp) {
     const Params P = *dp;
     CGS_PROLOGUE(W);
     ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, NP); return; }
     phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
-template <int W>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_residual(const Params* __restrict__ dp) {
+template <int W, int NP>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_init_residual(const Params* __restrict__ dp) {
     const Params P = *dp;
     CGS_PROLOGUE(W);
     if (warp >= W) return;
@@ -62,8 +62,8 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_residual(const 
     if (P.precond) { t = block_sum_w<W>(arz, rg.red); if (threadIdx.x == 0) P.part3[cta] = t; }
 }
 
-template <int W>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_scalars(const Params* __restrict__ dp) {
+template <int W, int NP>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_init_scalars(const Params* __restrict__ dp) {
     const Params P = *dp;
     CGS_PROLOGUE(W);
     if (warp >= W) return;
@@ -83,21 +83,21 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_init_scalars(const P
     }
 }
 
-template <int W, int U>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks1_spmv_dot(const Params* __restrict__ dp, int s) {
+template <int W, int NP, int U>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks1_spmv_dot(const Params* __restrict__ dp, int s) {
     const Params P = *dp;
     if (P.scal->st[s].stop) return;
     CGS_PROLOGUE(W);
     if (cta == 0 && threadIdx.x == 0) P.scal->brk[s] = 0;
     ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, kProducers); return; }
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, NP); return; }
     const double d = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, RingPos{0u, 0u, 0u});
     const double t = block_sum_w<W>(d, rg.red);
     if (threadIdx.x == 0) P.part0[cta] = t;
 }
 
-template <int W>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks2_update_xr(const Params* __restrict__ dp, int s) {
+template <int W, int NP>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks2_update_xr(const Params* __restrict__ dp, int s) {
     const Params P = *dp;
     if (P.scal->st[s].stop) return;
     CGS_PROLOGUE(W);
@@ -115,8 +115,8 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks2_update_xr(const Par
     if (P.precond) { t = block_sum_w<W>(arz, rg.red); if (threadIdx.x == 0) P.part2[cta] = t; }
 }
 
-template <int W>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks3_update_p(const Params* __restrict__ dp, int s) {
+template <int W, int NP>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks3_update_p(const Params* __restrict__ dp, int s) {
     const Params P = *dp;
     CGS_PROLOGUE(W);
     if (warp >= W) return;
@@ -159,11 +159,11 @@ __global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks3_update_p(const Para
 // R = 0: vectors in global memory (systems with more than R_max * 32 * W * G rows).
 // Scalars live in registers, identical in every CTA; three grid all-reduces per iteration
 // (after K1: p.q; after K2: r.r; after K3: a pure barrier that publishes p).
-template <int W, int U, int R, bool PRE>
-__global__ void __launch_bounds__(Shape<W>::kThreads, 1) ks_persistent(Params P) {
+template <int W, int NP, int U, int R, bool PRE>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Params P) {
     CGS_PROLOGUE(W);
     ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, LLONG_MAX, warp - W, kProducers); return; }
+    if (warp >= W) { producer_loop(P, rg, tb, Tc, LLONG_MAX, warp - W, NP); return; }
     const int lane = threadIdx.x & 31;
     const bool lead = cta == 0 && threadIdx.x == 0;
     Scal* S = P.scal;
