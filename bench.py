@@ -435,7 +435,7 @@ def main():
             # dram__bytes_read.sum + dram__bytes_write.sum of this launch (ks_persistent, one solve of 217
             # iterations of config 2) from profiles/r01_v2_ncu_full_raw_metrics.txt: the matrix comes
             # from DRAM once per solve, everything else is served by the L2
-            "traffic": 44.77e6 if (A.info("spmv") == 2 and A.info("loop") == 0) else None,
+            "traffic": 44.84e6 if (A.info("spmv") == 5 and A.info("loop") == 0) else None,
             "kernel": "ks_persistent (one launch = one solve)",
             "bytes_per_launch": bytes_it * it_per_solve + prologue_bytes,
             "peak_source": peak_src,
