@@ -125,8 +125,9 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               a shared-memory ring of 32-row tiles and W consumer warps with one lane per
  *               row and U entries in flight per lane: 2 = (W 12, 4 producers, U 9),
  *               3 = (8, 4, 27), 4 = (8, 4, 9), 5 = (11, 5, 9).  Auto picks 5 when the matrix is
- *               re-streamed from the L2 every iteration, else 2.  Falls back to 1 when a 32-row tile of the matrix does not fit
- *               a ring of 8 slots (227 KB of shared memory).
+ *               re-streamed from the L2 every iteration, else 2.  Falls back to 1 when a
+ *               32-row tile of the matrix does not fit a ring of 8 slots (227 KB of shared
+ *               memory), or for 5 when the ring depth is not a multiple of 5.
  *   "chunk"     iterations per graph replay in loop mode 1 (even, default 32)
  *   "resident"  1 (default) = the persistent streamed kernel keeps x, r, p, q in registers
  *               when every thread owns <= 4 rows; 0 = always in global memory
@@ -163,11 +164,14 @@ int cg_probe_read_bandwidth(cg_handle* h, const void* d_buf, size_t bytes, int r
                             double* h_gbs, void* cuda_stream);
 
 /* Phase trace of the persistent loop (loop mode 0), a profiling aid: with a non-NULL
- * d_trace (device uint64[grid * (iters + 1) * 16], grid = cg_get_info "grid"), thread 0 of every
- * CTA stores clock64() at 8 points (slots 0-7; slots 8-15 detail the third grid barrier) of each of the first `iters` iterations of later
- * solves: [0] iteration start, [1] K1 done, [2] past barrier 1, [3] K2 done, [4] past
- * barrier 2, [5] beta known, [6] K3 done, [7] past barrier 3.  Layout [cta][iter][slot].
- * NULL or iters = 0 switches it off (the default).  The buffer is borrowed. */
+ * d_trace (device uint64[grid * (iters + 1) * 16], grid = cg_get_info "grid"), thread 0 of
+ * every CTA stores clock64() at 8 points of each of the first `iters` iterations of later
+ * solves: [0] iteration start, [1] K1 done, [2] past all-reduce 1, [3] K2 done, [4] past
+ * all-reduce 2, [5] beta known, [6] K3 done, [7] past barrier 3; slots 8-15 detail that
+ * barrier.  Layout [cta][iter][slot]; row `iters` of every CTA holds ring statistics
+ * ([0] cycles producer warp 0 waited for free slots, [1] its lifetime, [2] tiles it issued,
+ * [3] cycles consumer thread 0 waited for data).  NULL or iters = 0 switches it off (the
+ * default).  The buffer is borrowed. */
 int cg_set_trace(cg_handle* h, uint64_t* d_trace, int64_t iters);
 
 /* Frees the host struct (and any CUDA graph).  Device memory is the caller's. */
