@@ -227,9 +227,8 @@ def main():
     ap.add_argument("--resident", type=int, default=None)
     ap.add_argument("--ring-slots", type=int, default=None)
     ap.add_argument("--fold", type=int, default=None)
-    ap.add_argument("--l2-hints", type=int, default=None)
-    ap.add_argument("--l2-prefetch", type=int, default=None)
     ap.add_argument("--pin", type=int, default=None)
+    ap.add_argument("--compress", type=int, default=None)
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -290,12 +289,10 @@ def main():
             Ap.set_option("ring_slots", args.ring_slots)
         if args.fold is not None:
             Ap.set_option("fold", args.fold)
-        if args.l2_hints is not None:
-            Ap.set_option("l2_hints", args.l2_hints)
-        if args.l2_prefetch is not None:
-            Ap.set_option("l2_prefetch", args.l2_prefetch)
         if args.pin is not None:
             Ap.set_option("pin", args.pin)
+        if args.compress is not None:
+            Ap.set_option("compress", args.compress)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []
@@ -311,7 +308,9 @@ def main():
             torch.cuda.synchronize()
             out.append(e0.elapsed_time(e1) * 1e3 / max(it, 1))
         rec = {"profile_config": args.profile, "iters": args.profile_iters, "us_per_iteration": out,
-               "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid")}
+               "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid"),
+               "compressed": Ap.info("compressed"), "pinned_tiles": Ap.info("pinned_tiles"),
+               "ring_slots": Ap.info("ring_slots"), "fold": Ap.info("fold"), "resident_rows": Ap.info("resident_rows")}
         if tr is not None:
             # [cta, iter, slot] clock64 stamps -> cycles per interval; skip the first 2 iterations
             full = tr.cpu().numpy().astype(np.int64)

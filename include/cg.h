@@ -21,11 +21,18 @@
  *    pinned host memory and, in graph mode, a CUDA graph).
  *  - CSR: 0-based int32 indices, rowptr[0] = 0, rowptr[n] = nnz, non-decreasing.
  *    Columns of a row need not be sorted or unique (duplicates add).
- *  - Return codes: 0 success / converged.  Positive = soft outcome of cg_solve:
- *    1 maxit reached, 2 breakdown (p.Ap <= 0 or not finite: A is not SPD).
+ *  - Return codes: 0 success / converged.  Positive = soft outcome: of cg_solve
+ *    1 maxit reached, 2 breakdown (p.Ap <= 0 or not finite: A is not SPD); of
+ *    cg_compress_index 3 (the index was left uncompressed).
  *    Negative = error: -1 invalid argument, -2 CUDA error (text via
- *    cg_strerror), -3 device not supported (needs compute capability 10.x).
+ *    cg_strerror), -3 device not supported (needs compute capability 10.x),
+ *    -4 device watchdog (a spin wait inside a solve ran out of its budget: a
+ *    protocol error or a lost copy; the results of that call are void, the device
+ *    is left usable), -5 out of host memory.
  *    Nothing is printed, thrown or aborted across this boundary.
+ *  - The sparsity structure (rowptr, colind) is fixed for the life of the handle;
+ *    vals may be rewritten between calls (then cg_set_option(h, "values_changed", 1)
+ *    so that cg_solve_jacobi extracts the diagonal again).
  *  - One handle per stream; concurrent calls on one handle are undefined.
  */
 #ifndef CG_B200_H
@@ -43,12 +50,15 @@ typedef struct cg_handle cg_handle;
 #define CG_OK             0
 #define CG_MAXIT          1
 #define CG_BREAKDOWN      2
+#define CG_NOTCOMPRESSED  3
 #define CG_EINVAL        -1
 #define CG_ECUDA         -2
 #define CG_EUNSUPPORTED  -3
+#define CG_ETIMEOUT      -4
+#define CG_ENOMEM        -5
 
 /* Bytes of device workspace cg_create needs for an n-row system: the vectors
- * r, p, q, D^-1 and one spare (each n doubles, 256-byte aligned), a padded copy of rowptr
+ * r, p, q, one spare and D^-1 (each n doubles, 256-byte aligned), a padded copy of rowptr
  * (n + 41 ints), the per-CTA reduction partials, the grid all-reduce inboxes (1.8 MB) and
  * the device-resident scalar state. */
 size_t cg_workspace_bytes(int64_t n);
@@ -64,6 +74,20 @@ int cg_create(cg_handle** out, int64_t n, int64_t nnz,
               const int32_t* d_rowptr, const int32_t* d_colind, const double* d_vals,
               void* d_workspace, size_t workspace_bytes);
 
+/* Optional compressed column index (the matrix comes "from
+ * a FEM model", so col - row takes few distinct values).  When the matrix has at most 256
+ * distinct offsets col - row, cg_compress_index builds, in caller-owned device memory, one
+ * record per 32-row tile (33 16-bit row starts + one byte per entry naming its offset) and the
+ * streamed kernels then move 9 instead of 12 bytes per entry: vals still come from the
+ * caller's array, in CSR order, so every result keeps its bits.  At the paper's size this
+ * makes each SM's slice of the matrix fit its shared memory for the whole solve.
+ * cg_index_bytes: size the buffer needs (0: not worth compressing, e.g. very uneven rows).
+ * cg_compress_index: d_index 256-byte aligned, borrowed until cg_destroy or the next call;
+ * returns CG_OK (in use from now on), CG_NOTCOMPRESSED (more than 256 offsets: nothing
+ * changes) or a negative error.  Synchronises the stream. */
+size_t cg_index_bytes(cg_handle* h);
+int cg_compress_index(cg_handle* h, void* d_index, size_t index_bytes, void* cuda_stream);
+
 /* Optional structural check of the bound CSR arrays on the device: rowptr[0] = 0,
  * rowptr[n] = nnz, non-decreasing, 0 <= colind < n.  Synchronises the stream.
  * Returns CG_OK or CG_EINVAL.  (Symmetry / definiteness are NOT checked:
@@ -75,7 +99,8 @@ int cg_check_csr(cg_handle* h, void* cuda_stream);
  * distinct buffers.  Asynchronous on the stream. */
 int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_stream);
 
-/* *h_result = sum_i a_i b_i (the p.Ap / r.r reductions of the CG loop), with a
+/* *h_result = sum_i a_i b_i (the p.Ap / r.r reductions of the CG loop, which PAPER.md:44
+ * counts among the "repetitive operations [that] run on GPU"), with a
  * fixed reduction order: bitwise reproducible run to run.  d_a, d_b: double[n].
  * Synchronises the stream once. */
 int cg_dot(cg_handle* h, const double* d_a, const double* d_b,
@@ -121,35 +146,47 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *                   with a device-side stop flag (the profilable twin)
  *               2 = plain per-iteration launches, same kernels as 1
  *   "spmv"      0 = auto; 1 = generic: sub-warp per row straight from global memory (any
- *               CSR matrix); 2.. = streamed: warp-specialised bulk-async (TMA) producers,
- *               a shared-memory ring of 32-row tiles and W consumer warps with one lane per
- *               row and U entries in flight per lane: 2 = (W 12, 4 producers, U 9),
- *               3 = (8, 4, 27), 4 = (8, 4, 9), 5 = (11, 5, 9).  Auto picks 5 when the matrix is
- *               re-streamed from the L2 every iteration, else 2.  Falls back to 1 when a
- *               32-row tile of the matrix does not fit a ring of 8 slots (227 KB of shared
- *               memory), or for 5 when the ring depth is not a multiple of 5.
+ *               CSR matrix); 2, 3, 4 = streamed: 32-row tiles in shared-memory slots filled by
+ *               bulk-async (TMA) copies, W consumer warps with one lane per row:
+ *               2 = 12 consumer + 4 producer warps, 9 entries in flight per lane, slots handed
+ *                   back to the producers before the gathers are issued;
+ *               3 = 11 + 5, likewise;
+ *               4 = 16 consumer warps and no producers (every warp copies its own tiles once),
+ *                   27 gathers in flight per lane: only when every CTA's slice of the matrix is
+ *                   pinned in shared memory (see "pin").
+ *               Auto picks 4 when everything is pinned, else 3 when the matrix is re-streamed
+ *               from the L2 every iteration or streams from HBM in compressed form, else 2.
+ *               A request that cannot run (a 32-row tile does not fit a ring of 8 slots in the
+ *               227 KB of shared memory; 4 without pinning) falls back to 1.
  *   "chunk"     iterations per graph replay in loop mode 1 (even, default 32)
  *   "resident"  1 (default) = the persistent streamed kernel keeps x, r, p, q in registers
  *               when every thread owns <= 4 rows; 0 = always in global memory
  *   "fold"      persistent streamed kernel with vectors in registers, no preconditioner:
  *               1 = fold K3 into the next K1 (every gathered p_j is recomputed on the fly as
- *               fma(beta, p_old_j, r_j), the owner's own expression, so results keep their
- *               bits) and synchronise the grid twice instead of three times per iteration;
- *               0 = off; 2 (default) = on when a CTA has <= 8 tiles (K1 is short)
- *   "l2_hints"  1 = evict_last / evict_first L2 hints on q between K1 and K2 when the matrix
- *               exceeds the L2 (default 0: measured a net loss, see cg_stream.cuh)
- *   "l2_prefetch" n > 0: producers prefetch n of their tiles (1 = 8) into the L2 ahead of the
- *               ring copies when the matrix exceeds the L2 (default 0: measured no gain)
- *   "pin"       1 (default) = when every CTA's slice of the matrix fits its ring (up to 64
- *               tiles in 225 KB of shared memory per SM), copy it there once per solve and
- *               keep it; 0 = stream everything every iteration
- *   "ring_slots" cap on the ring depth (8..64, rounded down to a multiple of 4)
+ *               fma(beta, p_old_j, r_j) from one 16-byte {p_old, r} pair, the owner's own
+ *               expression, so results keep their bits) and synchronise the grid twice
+ *               instead of three times per iteration; 0 = off; 2 (default) = on when a CTA has
+ *               <= 8 tiles or its whole slice of the matrix is pinned in shared memory
+ *   "pin"       1 (default) = when every CTA's slice of the matrix fits the shared memory (up
+ *               to 64 tiles per SM) and the matrix would otherwise be re-read from the L2 every
+ *               iteration, copy it there once per solve and keep it; 0 = stream everything
+ *               every iteration; k >= 2 = pin k tiles per CTA and stream the rest (a mixed
+ *               split, kept for tests and measurements)
+ *   "compress"  1 (default) = use the compressed index once cg_compress_index has built it;
+ *               0 = plain CSR slots
+ *   "ring_slots" cap on the ring depth (8..64)
  *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
  *               started (default unlimited: the ring is refilled across the grid barriers)
  *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant
+ *   "values_changed" (any value) the caller rewrote vals: cached D^-1 is dropped
+ *   "spin_budget_ms" how long any device-side spin may last before the watchdog trips and
+ *               the solve returns CG_ETIMEOUT (default 2000)
+ *   "inject_fault" tests only: k > 0 makes producer warp 0 of CTA 0 announce its k-th tile
+ *               and never copy it, which must end in CG_ETIMEOUT (default 0)
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
- * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "slot_bytes", "resident_rows".
+ * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "pinned_tiles", "slot_bytes",
+ * "resident_rows", "fold", "compressed", "index_codes", "from_hbm".
  * Unknown names return CG_EINVAL. */
 int cg_set_option(cg_handle* h, const char* name, int64_t value);
 int cg_get_info(cg_handle* h, const char* name, int64_t* value);

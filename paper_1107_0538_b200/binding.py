@@ -24,6 +24,8 @@ SIGNATURES = {
     "cg_workspace_bytes": (_sz, [_i64]),
     "cg_host_scratch_bytes": (_sz, [_i64, _i64]),
     "cg_create": (ctypes.c_int, [ctypes.POINTER(_vp), _i64, _i64, _vp, _vp, _vp, _vp, _sz]),
+    "cg_index_bytes": (_sz, [_vp]),
+    "cg_compress_index": (ctypes.c_int, [_vp, _vp, _sz, _vp]),
     "cg_check_csr": (ctypes.c_int, [_vp, _vp]),
     "cg_spmv": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "cg_dot": (ctypes.c_int, [_vp, _vp, _vp, ctypes.POINTER(_f64), _vp]),
@@ -93,6 +95,18 @@ def cg_create(n: int, nnz: int, d_rowptr: int, d_colind: int, d_vals: int,
 
 def cg_destroy(h: int) -> None:
     lib().cg_destroy(h)
+
+
+def cg_index_bytes(h: int) -> int:
+    return int(lib().cg_index_bytes(h))
+
+
+def cg_compress_index(h: int, d_index: int, index_bytes: int, stream: int = 0) -> int:
+    """Returns 0 (compressed index in use) or 3 (CG_NOTCOMPRESSED); raises on errors."""
+    rc = lib().cg_compress_index(h, d_index, index_bytes, stream)
+    if rc < 0:
+        raise CGError(rc, "cg_compress_index")
+    return rc
 
 
 def cg_check_csr(h: int, stream: int = 0) -> int:
@@ -184,7 +198,7 @@ class CGResult:
 class CG:
     """Handle bound to CSR arrays held in torch CUDA tensors (kept alive here)."""
 
-    def __init__(self, rowptr, colind, vals):
+    def __init__(self, rowptr, colind, vals, compress: bool = True):
         import torch
         if not (rowptr.is_cuda and colind.is_cuda and vals.is_cuda):
             raise ValueError("CSR arrays must be CUDA tensors (there is no CPU path)")
@@ -201,6 +215,20 @@ class CG:
         self.h = cg_create(self.n, self.nnz, self.rowptr.data_ptr(), self.colind.data_ptr(),
                            self.vals.data_ptr(), self.workspace.data_ptr(), wb)
         self._scratch = None
+        self.index = None
+        if compress:
+            self.compress()
+
+    def compress(self) -> bool:
+        """Build the compressed column index (cg_compress_index) in a tensor owned here.
+        Returns True when the handle now uses it."""
+        nb = cg_index_bytes(self.h)
+        if nb == 0:
+            return False
+        buf = self.torch.empty(nb, dtype=self.torch.uint8, device=self.device)
+        rc = cg_compress_index(self.h, buf.data_ptr(), nb, self._stream())
+        self.index = buf if rc == 0 else None
+        return rc == 0
 
     def close(self):
         if getattr(self, "h", None):

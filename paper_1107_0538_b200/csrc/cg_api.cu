@@ -8,6 +8,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include <new>
+#include <limits.h>
 
 using namespace cgk;
 
@@ -64,6 +65,91 @@ __global__ void k_diag_inv(Params P) {
             if (P.colind[k] == i) d += P.vals[k];
         if (!(d > 0.0) || !is_finite(d)) { P.scal->diag_bad = 1; d = 1.0; }
         P.dinv[i] = 1.0 / d;
+    }
+}
+
+// ---- cg_compress_index: setup kernels of the compressed column index (cg_stream.cuh).
+constexpr int kIdxHash = 1024;                       // open-addressing table of the distinct offsets col - row
+constexpr long long kIdxEmpty = LLONG_MIN;
+constexpr size_t kIdxTableOff = 0;                   // kMaxCodes ints: the sorted offsets
+constexpr size_t kIdxHashOff = 1024;                 // kIdxHash long longs of scratch
+constexpr size_t kIdxRecOff = 1024 + 8 * kIdxHash;   // records (a multiple of 128)
+
+// Pass 1: the set of distinct offsets d = col - row, at most kMaxCodes of them (else overflow).
+__global__ void k_idx_collect(const int* __restrict__ rowptr, const int* __restrict__ colind, long long n,
+                              long long* table, Scal* scal) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        if (*reinterpret_cast<volatile int*>(&scal->idx_overflow)) return;
+        long long last = kIdxEmpty;
+        for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+            const long long d = (long long)colind[k] - i;
+            if (d == last) continue;
+            last = d;
+            unsigned slot = (unsigned)((unsigned long long)d * 0x9E3779B97F4A7C15ULL >> 54);      // top 10 bits
+            int probes = 0;
+            for (;; slot = (slot + 1) & (kIdxHash - 1)) {
+                long long cur = table[slot];                     // a stale "empty" is settled by the CAS
+                if (cur == d) break;
+                if (cur == kIdxEmpty) {
+                    cur = (long long)atomicCAS(reinterpret_cast<unsigned long long*>(table + slot),
+                                               (unsigned long long)kIdxEmpty, (unsigned long long)d);
+                    if (cur == kIdxEmpty) {
+                        if (atomicAdd(&scal->idx_count, 1) + 1 > cgs::kMaxCodes) scal->idx_overflow = 1;
+                        break;
+                    }
+                    if (cur == d) break;
+                }
+                if (++probes >= kIdxHash) { scal->idx_overflow = 1; return; }
+            }
+        }
+    }
+}
+
+// Pass 2 (one CTA of kIdxHash threads): the offsets in ascending order -> codes 0 .. count - 1.
+__global__ void k_idx_sort(const long long* __restrict__ table, int* __restrict__ off) {
+    __shared__ long long keys[kIdxHash];
+    const long long mine = table[threadIdx.x];
+    keys[threadIdx.x] = mine;
+    if (threadIdx.x < cgs::kMaxCodes) off[threadIdx.x] = 0;
+    __syncthreads();
+    if (mine == kIdxEmpty) return;
+    int rank = 0;
+    for (int j = 0; j < kIdxHash; ++j) rank += (keys[j] != kIdxEmpty && keys[j] < mine) ? 1 : 0;
+    if (rank < cgs::kMaxCodes) off[rank] = (int)mine;
+}
+
+// Pass 3 (one warp per tile): the tile's record = 33 u16 row starts relative to the tile,
+// [33] = parity of the tile's first entry (the vals span starts at an even entry), then the
+// codes transposed: entry t of the tile's row l at byte 80 + 32 t + l.
+__global__ void k_idx_build(const int* __restrict__ rp_pad, const int* __restrict__ colind, long long n,
+                            const int* __restrict__ off, int ncodes, unsigned char* __restrict__ rec, int rec_stride) {
+    __shared__ int so[cgs::kMaxCodes];
+    for (int i = threadIdx.x; i < cgs::kMaxCodes; i += blockDim.x) so[i] = off[i];
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const long long ntiles = (n + kTileRows - 1) / kTileRows;
+    const long long wstride = (long long)gridDim.x * (blockDim.x >> 5);
+    const int maxlen = (rec_stride - cgs::kRecHdr) / 32;
+    for (long long t = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < ntiles; t += wstride) {
+        const long long row = t * kTileRows + lane;
+        const int s = rp_pad[t * kTileRows];
+        const int rs = rp_pad[row], re = rp_pad[row + 1];
+        unsigned char* r = rec + (size_t)t * (size_t)rec_stride;
+        unsigned short* hd = reinterpret_cast<unsigned short*>(r);
+        hd[lane] = (unsigned short)(rs - s);
+        if (lane < 8) hd[32 + lane] = lane == 0 ? (unsigned short)(rp_pad[t * kTileRows + kTileRows] - s)
+                                    : lane == 1 ? (unsigned short)(s & 1) : (unsigned short)0;
+        for (int tt = 0; tt < maxlen; ++tt) {
+            int code = 0;
+            if (tt < re - rs) {
+                const int d = (int)((long long)colind[rs + tt] - row);
+                int lo = 0, hi = ncodes - 1;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (so[mid] < d) lo = mid + 1; else hi = mid; }
+                code = lo;
+            }
+            r[cgs::kRecHdr + tt * 32 + lane] = (unsigned char)code;
+        }
     }
 }
 
@@ -222,9 +308,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_persistent(Params P) {
 
     // a0 prologue: q = A x0 ; r = b - q ; p = r ; rr, bb
     phase_spmv_vector_dispatch<false>(P, P.x, P.q, cta, G);
-    grid_barrier(&S->bar, G, epoch);
+    bool dead = grid_barrier(&S->bar, G, epoch, P.spin_budget, &S->abort);
     phase_init_residual(P, cta, G, sm);
-    grid_barrier(&S->bar, G, epoch);
+    dead = grid_barrier(&S->bar, G, epoch, P.spin_budget, &S->abort) || dead;
     double rr = sum_partials(P.part1, G, sm);
     const double bb = sum_partials(P.part2, G, sm);
     double rz = P.precond ? sum_partials(P.part3, G, sm) : rr;
@@ -232,6 +318,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_persistent(Params P) {
     long long k; int stop, status; double thresh;
     init_decide(P, rr, bb, &k, &stop, &status, &thresh);
     if (P.precond && S->diag_bad) { stop = 1; status = CG_BREAKDOWN; }
+    if (dead) { stop = 1; status = CG_ETIMEOUT; }
     if (lead && P.hist) P.hist[0] = sqrt(rr);
 
     // Optional trace (cg_set_trace): thread 0 of every CTA stamps clock64 at 8 points of each
@@ -247,7 +334,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_persistent(Params P) {
         const double t = block_sum(d, sm);
         if (threadIdx.x == 0) P.part0[cta] = t;
         CG_STAMP(1);
-        grid_barrier(&S->bar, G, epoch);
+        if (grid_barrier(&S->bar, G, epoch, P.spin_budget, &S->abort)) { stop = 1; status = CG_ETIMEOUT; break; }
         CG_STAMP(2);
         // scalar alpha (every CTA, same order, same value)
         const double pq = sum_partials(P.part0, G, sm);
@@ -256,7 +343,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_persistent(Params P) {
         // K2
         phase_update_xr<2>(P, alpha, cta, G, sm);
         CG_STAMP(3);
-        grid_barrier(&S->bar, G, epoch);
+        if (grid_barrier(&S->bar, G, epoch, P.spin_budget, &S->abort)) { stop = 1; status = CG_ETIMEOUT; break; }
         CG_STAMP(4);
         // scalar beta, continue-condition
         const double rr_new = sum_partials(P.part1, G, sm);
@@ -272,9 +359,10 @@ __global__ void __launch_bounds__(kThreads, 2) k_persistent(Params P) {
         // K3
         phase_update_p<2>(P, beta, cta, G);
         CG_STAMP(6);
-        grid_barrier(&S->bar, G, epoch);
+        dead = grid_barrier(&S->bar, G, epoch, P.spin_budget, &S->abort);
         CG_STAMP(7);
         k += 1;
+        if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
     }
 #undef CG_STAMP
     if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(rr); }
@@ -299,41 +387,61 @@ static thread_local char g_cuda_err[256] = "no CUDA error recorded";
         }                                                                     \
     } while (0)
 
-// Streamed variants: W consumer warps, U entries in flight per lane (cg_stream.cuh).
-// "spmv" option value = index + 2.
+// Streamed variants: W consumer warps, NP producer warps, U entries in flight per lane
+// (cg_stream.cuh).  "spmv" option value = index + 2.  Every kernel that touches the ring exists
+// for both slot formats ([cmp]: 0 plain CSR, 1 compressed index).
+enum PersistentKind { kR0, kR0Jacobi, kR2, kR2Jacobi, kR2Fold, kR4, kR4Jacobi, kR4Fold, kNumPersistent };
 struct StreamFns {
     int W, NP, U;
-    const void* spmv;
-    const void* init_spmv; const void* init_residual; const void* init_scalars;
-    const void* k1; const void* k2; const void* k3;
-    const void* persistent[3][2];          // [R index: 0 -> global vectors, 1 -> R = 2, 2 -> R = 4][Jacobi]
+    const void* spmv[2];
+    const void* init_spmv[2]; const void* init_residual; const void* init_scalars;
+    const void* k1[2]; const void* k2; const void* k3;
+    const void* persistent[2][kNumPersistent];
 };
 
-template <int W, int NP, int U> static StreamFns make_stream_fns() {
+template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(StreamFns& f) {
+    constexpr int c = CMP ? 1 : 0;
+    f.spmv[c] = (const void*)cgs::ks_spmv<W, NP, U, GF, CMP>;
+    f.init_spmv[c] = (const void*)cgs::ks_init_spmv<W, NP, U, GF, CMP>;
+    f.k1[c] = (const void*)cgs::ks1_spmv_dot<W, NP, U, GF, CMP>;
+    f.persistent[c][kR0]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 0, false, false, CMP>;
+    f.persistent[c][kR0Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 0, true, false, CMP>;
+    f.persistent[c][kR2]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 2, false, false, CMP>;
+    f.persistent[c][kR2Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 2, true, false, CMP>;
+    f.persistent[c][kR2Fold]   = (const void*)cgs::ks_persistent<W, NP, U, GF, 2, false, true, CMP>;
+    f.persistent[c][kR4]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, false, CMP>;
+    f.persistent[c][kR4Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, true, false, CMP>;
+    f.persistent[c][kR4Fold]   = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, true, CMP>;
+}
+template <int W, int NP, int U, bool GF> static StreamFns make_stream_fns() {
     StreamFns f;
     f.W = W; f.NP = NP; f.U = U;
-    f.spmv = (const void*)cgs::ks_spmv<W, NP, U>;
-    f.init_spmv = (const void*)cgs::ks_init_spmv<W, NP, U>;
     f.init_residual = (const void*)cgs::ks_init_residual<W, NP>;
     f.init_scalars = (const void*)cgs::ks_init_scalars<W, NP>;
-    f.k1 = (const void*)cgs::ks1_spmv_dot<W, NP, U>;
     f.k2 = (const void*)cgs::ks2_update_xr<W, NP>;
     f.k3 = (const void*)cgs::ks3_update_p<W, NP>;
-    f.persistent[0][0] = (const void*)cgs::ks_persistent<W, NP, U, 0, false>;
-    f.persistent[0][1] = (const void*)cgs::ks_persistent<W, NP, U, 0, true>;
-    f.persistent[1][0] = (const void*)cgs::ks_persistent<W, NP, U, 2, false>;
-    f.persistent[1][1] = (const void*)cgs::ks_persistent<W, NP, U, 2, true>;
-    f.persistent[2][0] = (const void*)cgs::ks_persistent<W, NP, U, 4, false>;
-    f.persistent[2][1] = (const void*)cgs::ks_persistent<W, NP, U, 4, true>;
+    fill_cmp_fns<W, NP, U, GF, false>(f);
+    fill_cmp_fns<W, NP, U, GF, true>(f);
     return f;
 }
-static constexpr int kNumStream = 4;
+static constexpr int kNumStream = 3;
 static const StreamFns& stream_fns(int idx) {
-    static const StreamFns table[kNumStream] = {
-        make_stream_fns<12, 4, 9>(), make_stream_fns<8, 4, 27>(), make_stream_fns<8, 4, 9>(),
-        make_stream_fns<11, 5, 9>()};
+    static const StreamFns table[kNumStream] = {make_stream_fns<12, 4, 9, false>(), make_stream_fns<11, 5, 9, false>(),
+                                                make_stream_fns<16, 0, 27, true>()};
     return table[idx];
 }
+
+// Ring geometry and pinning of one launch configuration (a function of the handle's matrix
+// statistics, its options and whether the compressed index is in use).
+struct Geo {
+    bool valid;                 // the streamed kernels can run this matrix
+    int cmp;                    // slot format
+    int cap, slot_bytes, rec_stride;
+    int slots;                  // S = pinned + stream_slots (+ unused remainder)
+    int pinned, stream_slots;   // P, Q
+    bool from_hbm;              // the matrix stream exceeds half the L2
+    size_t smem;
+};
 
 struct cg_handle {
     long long n, nnz;
@@ -343,19 +451,19 @@ struct cg_handle {
     int* rp_pad;
     Scal* scal; Params* dparams;
     Scal* h_scal; Params* h_params;        // pinned host mirrors
-    int sms, smem_optin;
+    int sms, smem_optin, clock_khz;
     size_t l2_bytes;
-    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, l2_hints, l2_prefetch, pin_opt;
+    int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, pin_opt, compress_opt;
+    int spin_budget_ms, inject_fault;
     int max_row_len, max_tile_nnz, tpr;
     bool dinv_ready;
     int grid_generic;                      // cooperative grid of the generic variant
-    int cap, slots, slot_bytes;            // ring geometry of the streamed variants
-    bool stream_ok[kNumStream];
-    cudaGraphExec_t gexec; int gexec_variant, gexec_chunk, gexec_grid;
+    unsigned char* idx; size_t idx_bytes; bool idx_ready; int idx_codes;     // compressed index (borrowed buffer)
+    cudaGraphExec_t gexec; int gexec_variant, gexec_chunk, gexec_grid, gexec_cmp; size_t gexec_smem;
     cudaStream_t cap_stream;               // capture-only stream (the legacy stream cannot capture)
     unsigned long long* trace; int trace_iters;
     long long launches;
-    int last_resident;                     // R used by the last persistent solve (info)
+    int last_resident, last_fold;          // what the last persistent solve used (info)
 };
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -378,8 +486,6 @@ extern "C" size_t cg_host_scratch_bytes(int64_t n, int64_t maxit) {
     return 2 * vec_bytes(n) + align_up((size_t)(maxit + 1) * 8u, 256);
 }
 
-static size_t stream_smem(const cg_handle* h) { return (size_t)h->slots * h->slot_bytes + cgs::kSmemTail; }
-
 static int setup_generic(cg_handle* h) {
     int bps = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_persistent, kThreads, 0));
@@ -392,55 +498,111 @@ static int setup_generic(cg_handle* h) {
     return CG_OK;
 }
 
-// Ring geometry from the matrix statistics; the streamed variants need a ring of at least
-// 8 slots in the opt-in shared memory, in a number the variant's producer count divides.
-static int setup_stream(cg_handle* h) {
-    h->cap = (h->max_tile_nnz + 6 + 3) & ~3;
-    if (h->cap < 4) h->cap = 4;
-    h->slot_bytes = (int)align_up((size_t)h->cap * 12u + (size_t)cgs::kRpInts * 4u, 128);
-    const long long budget = (long long)h->smem_optin - cgs::kSmemTail;
-    long long S = budget / h->slot_bytes;
-    if (S > cgs::kMaxSlots) S = cgs::kMaxSlots;
-    if (S > h->max_slots) S = h->max_slots;
-    // A slot must always be refilled by the same producer warp (tile j -> warp j mod NP, slot
-    // j mod S): otherwise a warp could run two phases ahead of a slot's "empty" barrier, which
-    // a parity wait cannot tell from zero phases ahead.  So NP must divide S: multiples of 20
-    // serve both producer counts (4 and 5), shallower rings only the variants with 4.
-    S -= S % (S >= cgs::kSlotQuantum ? cgs::kSlotQuantum : 4);
-    h->slots = (int)S;
-    for (int v = 0; v < kNumStream; ++v) {
-        const StreamFns& f = stream_fns(v);
-        h->stream_ok[v] = S >= 8 && S % f.NP == 0 && h->sms <= cgs::kBarGrid;   // slots are released early: S need not cover W
-        if (!h->stream_ok[v]) continue;
-        const int smem = h->smem_optin;      // the attribute is per function, not per handle: always the maximum
-        const void* fns[] = {f.spmv, f.init_spmv, f.init_residual, f.init_scalars, f.k1, f.k2, f.k3,
-                             f.persistent[0][0], f.persistent[0][1], f.persistent[1][0],
-                             f.persistent[1][1], f.persistent[2][0], f.persistent[2][1]};
-        for (const void* fn : fns)
-            CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+static long long tiles_per_cta_max(const cg_handle* h) {
+    return ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
+}
+static int rec_stride_of(const cg_handle* h) { return (int)align_up((size_t)cgs::kRecHdr + 32u * (size_t)h->max_row_len, 16); }
+static bool use_cmp(const cg_handle* h) { return h->idx_ready && h->compress_opt != 0; }
+
+// Ring geometry of streamed variant `idx` from the matrix statistics.  A slot holds the largest
+// tile: plain CSR cap * 12 + 144 bytes (cap = max tile nnz widened by the 16-byte alignment of
+// the colind span), compressed cap * 8 + record bytes.  Pinning (option "pin": 1 = auto,
+// 0 = never, k >= 2 = pin k tiles per CTA and stream the rest, for tests): when the matrix is
+// re-read from the L2 every iteration anyway and every CTA's slice fits the shared memory, the
+// ring is exactly the slice and nothing streams.  Otherwise the tiles stream through a ring
+// whose depth Q is a multiple of the variant's producer count NP: a slot must always be
+// refilled by the same producer warp (tile j -> warp j mod NP, slot j mod Q), otherwise a warp
+// could run two phases ahead of a slot's "empty" barrier, which a parity wait cannot tell from
+// zero phases ahead.  A variant without producer warps (NP = 0) needs everything pinned.
+static Geo geometry(const cg_handle* h, bool cmp, int idx) {
+    Geo g; memset(&g, 0, sizeof(g));
+    const int NP = stream_fns(idx).NP;
+    g.cmp = cmp ? 1 : 0;
+    g.rec_stride = rec_stride_of(h);
+    if (cmp) {
+        g.cap = (h->max_tile_nnz + 2 + 1) & ~1;
+        g.slot_bytes = (int)align_up((size_t)g.cap * 8u + (size_t)g.rec_stride, 16);
+    } else {
+        g.cap = (h->max_tile_nnz + 6 + 3) & ~3;
+        if (g.cap < 4) g.cap = 4;
+        g.slot_bytes = (int)align_up((size_t)g.cap * 12u + (size_t)cgs::kRpInts * 4u, 128);
     }
-    return CG_OK;
+    const size_t fixed = (size_t)cgs::kSmemTail + (cmp ? (size_t)cgs::kOffTabBytes : 0u);
+    long long raw = ((long long)h->smem_optin - (long long)fixed) / g.slot_bytes;
+    if (raw > cgs::kMaxSlots) raw = cgs::kMaxSlots;
+    if (raw > h->max_slots) raw = h->max_slots;
+    const long long tc_max = tiles_per_cta_max(h);
+    g.from_hbm = (size_t)h->nnz * (cmp ? 9u : 12u) > h->l2_bytes / 2;
+    if (h->sms > cgs::kBarGrid || raw < 1) return g;
+    if (h->pin_opt == 1 && !g.from_hbm && tc_max <= raw) {
+        g.slots = (int)tc_max; g.pinned = (int)tc_max; g.stream_slots = 0; g.valid = true;
+    } else if (NP > 0) {
+        long long P = h->pin_opt >= 2 ? (h->pin_opt < tc_max ? h->pin_opt : tc_max) : 0;
+        if (P > raw - 8) P = raw - 8 > 0 ? raw - 8 : 0;
+        long long Q = raw - P;
+        Q -= Q % NP;
+        g.pinned = (int)P; g.stream_slots = (int)Q; g.slots = (int)(P + Q);
+        g.valid = Q >= 8;                   // slots are released early: the ring need not cover the consumer warps
+    }
+    g.smem = (size_t)g.slots * g.slot_bytes + fixed;
+    return g;
 }
 
-// 1 = generic; 2 + i = streamed variant i.  Auto: 12 consumer + 4 producer warps when the matrix
-// streams from HBM (config 4) or is pinned in shared memory (configs 0, 1: the producers
-// idle); 11 + 5 when it is re-streamed from the L2 every iteration (configs 2, 3: measured
-// 13.40 -> 12.68 and 34.28 -> 34.13 us per iteration; 292 -> 295 at config 4, 16.4 -> 17.2 at
-// config 1).
-static int pick_variant(const cg_handle* h) {
-    if (h->spmv_opt == 1) return 1;
-    if (h->spmv_opt >= 2) return h->stream_ok[h->spmv_opt - 2] ? h->spmv_opt : 1;
-    const long long tc_max = ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
-    const bool from_hbm = (size_t)h->nnz * 12u > h->l2_bytes / 2;
-    const bool pinned = h->pin_opt && !from_hbm && tc_max <= h->slots;
-    if (!from_hbm && !pinned && h->stream_ok[3]) return 5;
-    return h->stream_ok[0] ? 2 : 1;
+// 1 = generic; 2 + i = streamed variant i.  Auto:
+//   everything pinned in shared memory       16 consumer warps, no producers, 27 gathers in flight
+//   re-streamed from the L2 every iteration  11 consumer + 5 producer warps (configs 2, 3 in round
+//                                            1: 13.40 -> 12.68 and 34.28 -> 34.13 us per iteration)
+//   streamed from HBM                        11 + 5 with the compressed index (two copies per tile,
+//                                            config 4: 254 against 276 us per iteration), 12 + 4 with
+//                                            plain CSR slots (292 against 295)
+static int pick_variant(const cg_handle* h, Geo* out = nullptr) {
+    const bool cmp = use_cmp(h);
+    Geo g; memset(&g, 0, sizeof(g));
+    int v = 1;
+    if (h->spmv_opt >= 2) {
+        g = geometry(h, cmp, h->spmv_opt - 2);
+        v = g.valid ? h->spmv_opt : 1;
+    } else if (h->spmv_opt == 0) {
+        const Geo g2 = geometry(h, cmp, 2);
+        if (g2.valid) { g = g2; v = 4; }
+        else {
+            const Geo g1 = geometry(h, cmp, 1), g0 = geometry(h, cmp, 0);
+            const bool five = g1.valid && (!g1.from_hbm || cmp);
+            if (five) { g = g1; v = 3; }
+            else if (g0.valid) { g = g0; v = 2; }
+            else if (g1.valid) { g = g1; v = 3; }
+        }
+    }
+    if (v == 1) { g = geometry(h, cmp, 0); }
+    if (out) *out = g;
+    return v;
 }
 
 static int variant_grid(const cg_handle* h, int v) { return v == 1 ? h->grid_generic : h->sms; }
 
+// Rows per consumer thread the persistent kernel would keep in registers (0: global vectors).
+static int resident_rows(const cg_handle* h, int v) {
+    if (v < 2 || !h->resident_opt) return 0;
+    const int W = stream_fns(v - 2).W;
+    const long long need = (tiles_per_cta_max(h) + W - 1) / W;
+    return need <= 2 ? 2 : need <= 4 ? 4 : 0;        // 8 rows per thread spill and gain nothing (measured on config 1)
+}
+
+// Folding K3 into the next K1 trades a grid synchronisation for a 16-byte gather per entry
+// instead of an 8-byte one.  Option "fold": 0 off, 1 on, 2 auto.
+static bool fold_effective(const cg_handle* h, int v, int precond, const Geo& g) {
+    if (precond || resident_rows(h, v) == 0) return false;
+    if (h->fold_opt != 2) return h->fold_opt == 1;
+    // auto: the 16-byte gathers must cost less than the synchronisation they save.  Measured
+    // (us per iteration, folded / not): config 0 (1 tile of 24 entries per row per CTA) 7.4 / 7.8,
+    // config 1 (56 pinned tiles x 7) 10.6 / 13.4, config 2 (29 pinned tiles x 26) 10.8 / 10.4.
+    const double gathers = (double)tiles_per_cta_max(h) * (double)h->nnz / (double)h->n;
+    return gathers <= 500.0;
+}
+
 static void fill_params(const cg_handle* h, Params* P, const double* b, double* x, double rtol,
-                        long long maxit, double* hist, int precond, int variant) {
+                        long long maxit, double* hist, int precond, int variant, const Geo& g) {
+    memset(P, 0, sizeof(*P));
     P->n = h->n; P->nnz = h->nnz;
     P->rowptr = h->rowptr; P->colind = h->colind; P->vals = h->vals;
     P->b = b; P->x = x; P->r = h->r; P->p = h->p; P->q = h->q; P->dinv = h->dinv;
@@ -449,28 +611,19 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     P->precond = precond; P->spmv = variant; P->tpr = h->tpr;
     P->trace = h->trace; P->trace_iters = h->trace_iters;
     P->rp_pad = h->rp_pad; P->bslots = h->bslots;
-    P->cap = h->cap; P->slots = h->slots; P->slot_bytes = h->slot_bytes;
+    P->cap = g.cap; P->slots = g.slots; P->slot_bytes = g.slot_bytes;
+    P->pinned = g.pinned; P->stream_slots = g.stream_slots;
     P->lookahead = h->lookahead;
-    P->l2_prefetch = h->l2_prefetch;
-    P->p2 = h->spare;
-    // Folding K3 into the next K1 trades a grid synchronisation for a second gather per entry:
-    // measured a gain only while K1 is short (<= 8 tiles per CTA), a loss when gathers are
-    // irregular (config 3: 38 -> 60 us per iteration).  2 = auto.
-    const long long tc_max = ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
-    P->fold = h->fold_opt == 2 ? (tc_max <= 8 ? 1 : 0) : h->fold_opt;
-    P->l2_stream = ((size_t)h->nnz * 12u > h->l2_bytes / 2) ? (h->l2_hints ? 3 : 1) : 0;
-    // Pinned tiles (cg_stream.cuh): when every CTA's slice of the matrix fits the ring, it is
-    // copied into shared memory once per solve and stays there.
-    P->pinned = 0; P->stream_slots = h->slots;
-    if (h->pin_opt && !P->l2_stream && variant >= 2) {
-        if (tc_max <= h->slots) {
-            P->pinned = (int)tc_max;
-            P->stream_slots = (h->slots - (int)tc_max) / cgs::kSlotQuantum * cgs::kSlotQuantum;   // unused: nothing streams
-        }
-        // A partial split (pin S - 8 tiles, stream the rest through 8 slots) was measured on
-        // config 2 and lost: K1 12.4 k against 10.2 k cycles, the streamed tiles queue up
-        // behind too few slots.  The kernels support it; the host never asks for it.
-    }
+    // the pair buffers of the folded loop reuse {r, p} and {q, spare}: with the vectors in
+    // registers (the only case that folds) none of the four is used otherwise
+    P->pr0 = reinterpret_cast<double2*>(h->r);
+    P->pr1 = reinterpret_cast<double2*>(h->q);
+    P->l2_stream = g.from_hbm ? 1 : 0;
+    P->cmp = g.cmp; P->rec_stride = g.rec_stride;
+    P->idx_off = h->idx ? reinterpret_cast<const int*>(h->idx + kIdxTableOff) : nullptr;
+    P->idx_rec = h->idx ? h->idx + kIdxRecOff : nullptr;
+    P->spin_budget = (long long)h->spin_budget_ms * (long long)h->clock_khz;
+    P->inject_fault = h->inject_fault;
 }
 
 extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
@@ -489,20 +642,22 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, dev));
     if (prop.major != 10) return CG_EUNSUPPORTED;
-    int coop = 0;
+    int coop = 0, khz = 0;
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     if (!coop) return CG_EUNSUPPORTED;
+    CK(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
 
     cg_handle* h = new (std::nothrow) cg_handle();
-    if (!h) return CG_EINVAL;
+    if (!h) return CG_ENOMEM;
     memset(h, 0, sizeof(*h));
     h->n = n; h->nnz = nnz;
     h->rowptr = d_rowptr; h->colind = d_colind; h->vals = d_vals;
     h->ws = static_cast<unsigned char*>(d_workspace); h->ws_bytes = workspace_bytes;
     unsigned char* w = h->ws;
     const size_t vb = vec_bytes(n);
+    // r | p and q | spare are adjacent on purpose: each pair of vectors doubles as one {p, r} pair buffer
     h->r = (double*)w; w += vb; h->p = (double*)w; w += vb; h->q = (double*)w; w += vb;
-    h->dinv = (double*)w; w += vb; h->spare = (double*)w; w += vb;
+    h->spare = (double*)w; w += vb; h->dinv = (double*)w; w += vb;
     h->rp_pad = (int*)w; w += rp_pad_bytes(n);
     h->part0 = (double*)w; w += kPartBytes; h->part1 = (double*)w; w += kPartBytes;
     h->part2 = (double*)w; w += kPartBytes; h->part3 = (double*)w; w += kPartBytes;
@@ -511,8 +666,11 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     static_assert(sizeof(Scal) <= kScalBytes && sizeof(Params) <= kParamBytes, "workspace slots");
     h->sms = prop.multiProcessorCount;
     h->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    h->clock_khz = khz > 0 ? khz : 2000000;
     h->l2_bytes = (size_t)prop.l2CacheSize;
-    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1; h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->l2_hints = 0; h->l2_prefetch = 0; h->pin_opt = 1;
+    h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1;
+    h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->pin_opt = 1; h->compress_opt = 1;
+    h->spin_budget_ms = 2000; h->inject_fault = 0;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_params, sizeof(Params), cudaHostAllocDefault);
@@ -537,8 +695,19 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     const double mean = (double)nnz / (double)n;
     h->tpr = mean <= 3 ? 2 : mean <= 6 ? 4 : mean <= 40 ? 8 : mean <= 96 ? 16 : 32;
     int rc = setup_generic(h);
-    if (rc == CG_OK) rc = setup_stream(h);
     if (rc != CG_OK) { cg_destroy(h); return rc; }
+    // the opt-in shared-memory size is a per-function attribute: always the maximum
+    for (int v = 0; v < kNumStream; ++v) {
+        const StreamFns& f = stream_fns(v);
+        const void* one[] = {f.init_residual, f.init_scalars, f.k2, f.k3};
+        for (const void* fn : one) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
+        for (int c = 0; c < 2; ++c) {
+            const void* two[] = {f.spmv[c], f.init_spmv[c], f.k1[c]};
+            for (const void* fn : two) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
+            for (int k = 0; k < kNumPersistent; ++k)
+                CKH(cudaFuncSetAttribute(f.persistent[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
+        }
+    }
     *out = h;
     return CG_OK;
 }
@@ -558,35 +727,92 @@ extern "C" const char* cg_strerror(int code) {
         case CG_OK: return "success / converged";
         case CG_MAXIT: return "maximum number of iterations reached";
         case CG_BREAKDOWN: return "breakdown: p.Ap <= 0 or not finite (matrix not SPD)";
+        case CG_NOTCOMPRESSED: return "index not compressed: more than 256 distinct column offsets, or not worth it";
         case CG_EINVAL: return "invalid argument";
         case CG_ECUDA: return g_cuda_err;
         case CG_EUNSUPPORTED: return "device not supported (needs compute capability 10.x with cooperative launch)";
+        case CG_ETIMEOUT: return "device watchdog: a spin wait inside the solve exceeded its budget; results are void";
+        case CG_ENOMEM: return "out of host memory";
         default: return "unknown code";
     }
 }
 
+// ---- compressed column index
+
+// Bytes of the index buffer: offset table, hash scratch, one record per tile.  0 when the
+// matrix is not worth compressing: the records are ELL inside a tile (32 x longest row), so
+// a matrix with very uneven rows would make them larger than the 4 bytes per entry they replace.
+extern "C" size_t cg_index_bytes(cg_handle* h) {
+    if (!h || h->nnz == 0 || h->max_row_len == 0 || h->max_tile_nnz > 65535) return 0;
+    const size_t ntiles = (size_t)((h->n + kTileRows - 1) / kTileRows);
+    const size_t rec = ntiles * (size_t)rec_stride_of(h);
+    if (rec > 2u * (size_t)h->nnz + (1u << 20)) return 0;
+    return align_up(kIdxRecOff + rec, 256);
+}
+
+extern "C" int cg_compress_index(cg_handle* h, void* d_index, size_t index_bytes, void* cuda_stream) {
+    if (!h) return CG_EINVAL;
+    h->idx_ready = false; h->idx = nullptr; h->idx_bytes = 0; h->idx_codes = 0;
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    const size_t need = cg_index_bytes(h);
+    if (need == 0) return CG_NOTCOMPRESSED;
+    if (!d_index || (reinterpret_cast<uintptr_t>(d_index) & 255u) || index_bytes < need) return CG_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* idx = static_cast<unsigned char*>(d_index);
+    long long* table = reinterpret_cast<long long*>(idx + kIdxHashOff);
+    int* off = reinterpret_cast<int*>(idx + kIdxTableOff);
+    CK(cudaMemsetAsync(&h->scal->idx_count, 0, 2 * sizeof(int), st));
+    {   // LLONG_MIN in every hash slot
+        static_assert(kIdxEmpty == LLONG_MIN, "empty key");
+        long long* hinit = static_cast<long long*>(malloc(sizeof(long long) * kIdxHash));
+        if (!hinit) return CG_ENOMEM;
+        for (int i = 0; i < kIdxHash; ++i) hinit[i] = kIdxEmpty;
+        cudaError_t e = cudaMemcpyAsync(table, hinit, sizeof(long long) * kIdxHash, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        free(hinit);
+        CK(e);
+    }
+    k_idx_collect<<<h->sms * 8, 256, 0, st>>>(h->rowptr, h->colind, h->n, table, h->scal);
+    CK(cudaGetLastError());
+    k_idx_sort<<<1, kIdxHash, 0, st>>>(table, off);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(h->h_scal, h->scal, sizeof(Scal), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    h->launches = 2;
+    if (h->h_scal->idx_overflow || h->h_scal->idx_count > cgs::kMaxCodes || h->h_scal->idx_count < 1)
+        return CG_NOTCOMPRESSED;
+    const int ncodes = h->h_scal->idx_count;
+    k_idx_build<<<h->sms * 8, 256, 0, st>>>(h->rp_pad, h->colind, h->n, off, ncodes, idx + kIdxRecOff, rec_stride_of(h));
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
+    h->launches = 3;
+    h->idx = idx; h->idx_bytes = index_bytes; h->idx_codes = ncodes; h->idx_ready = true;
+    return CG_OK;
+}
+
 extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!h || !name) return CG_EINVAL;
+    auto drop_graph = [&]() { if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; } };
     if (!strcmp(name, "loop")) { if (value < 0 || value > 2) return CG_EINVAL; h->loop = (int)value; return CG_OK; }
     if (!strcmp(name, "spmv")) { if (value < 0 || value > 1 + kNumStream) return CG_EINVAL; h->spmv_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "chunk")) { if (value < 2 || value > 4096 || (value & 1)) return CG_EINVAL; h->chunk = (int)value; return CG_OK; }
     if (!strcmp(name, "lookahead")) { if (value < 0 || value > (1 << 30)) return CG_EINVAL; h->lookahead = (int)value; return CG_OK; }
     if (!strcmp(name, "ring_slots")) {
         if (value < 8 || value > cgs::kMaxSlots) return CG_EINVAL;
-        h->max_slots = (int)value;
-        if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // captured with the old smem size
-        return setup_stream(h);
-    }
-    if (!strcmp(name, "pin")) {
-        if (value < 0 || value > 1) return CG_EINVAL;
-        h->pin_opt = (int)value;
-        if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }      // kernels read it from Params, but be safe
+        h->max_slots = (int)value; drop_graph();
         return CG_OK;
     }
-    if (!strcmp(name, "l2_prefetch")) { if (value < 0 || value > 32) return CG_EINVAL; h->l2_prefetch = (int)value; return CG_OK; }
-    if (!strcmp(name, "l2_hints")) { if (value < 0 || value > 1) return CG_EINVAL; h->l2_hints = (int)value; return CG_OK; }
+    if (!strcmp(name, "pin")) {
+        if (value < 0 || value > cgs::kMaxSlots) return CG_EINVAL;
+        h->pin_opt = (int)value; drop_graph();
+        return CG_OK;
+    }
+    if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
+    if (!strcmp(name, "spin_budget_ms")) { if (value < 1 || value > 600000) return CG_EINVAL; h->spin_budget_ms = (int)value; return CG_OK; }
+    if (!strcmp(name, "inject_fault")) { if (value < 0 || value > (1 << 30)) return CG_EINVAL; h->inject_fault = (int)value; return CG_OK; }
+    if (!strcmp(name, "values_changed")) { h->dinv_ready = false; return CG_OK; }
     if (!strcmp(name, "tpr")) {
         if (value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return CG_EINVAL;
         h->tpr = (int)value; return CG_OK;
@@ -599,36 +825,32 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     return CG_EINVAL;
 }
 
-// Rows per consumer thread the persistent kernel would keep in registers (0: global vectors).
-static int resident_rows(const cg_handle* h, int v) {
-    if (v < 2 || !h->resident_opt) return 0;
-    const long long ntiles = (h->n + kTileRows - 1) / kTileRows;
-    const long long tc_max = (ntiles + h->sms - 1) / h->sms;
-    const int W = stream_fns(v - 2).W;
-    const long long need = (tc_max + W - 1) / W;
-    return need <= 2 ? 2 : need <= 4 ? 4 : 0;        // 8 rows per thread spill and gain nothing (measured on config 1)
-}
-
 extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     if (!h || !name || !value) return CG_EINVAL;
-    const int v = pick_variant(h);
+    Geo g;
+    const int v = pick_variant(h, &g);
     if (!strcmp(name, "loop")) *value = h->loop;
     else if (!strcmp(name, "spmv")) *value = v;
     else if (!strcmp(name, "grid")) *value = variant_grid(h, v);
     else if (!strcmp(name, "block")) *value = v == 1 ? kThreads : 32 * (stream_fns(v - 2).W + stream_fns(v - 2).NP);
-    else if (!strcmp(name, "smem")) *value = (int64_t)(v >= 2 ? stream_smem(h) : 0);
+    else if (!strcmp(name, "smem")) *value = (int64_t)(v >= 2 ? g.smem : 0);
     else if (!strcmp(name, "launches")) *value = h->launches;
     else if (!strcmp(name, "sms")) *value = h->sms;
     else if (!strcmp(name, "tpr")) *value = h->tpr;
     else if (!strcmp(name, "max_row_len")) *value = h->max_row_len;
     else if (!strcmp(name, "max_tile_nnz")) *value = h->max_tile_nnz;
-    else if (!strcmp(name, "stream_ok")) *value = h->stream_ok[0] ? 1 : 0;
+    else if (!strcmp(name, "stream_ok")) *value = geometry(h, use_cmp(h), 0).valid ? 1 : 0;
     else if (!strcmp(name, "consumer_warps")) *value = v >= 2 ? stream_fns(v - 2).W : 0;
     else if (!strcmp(name, "producer_warps")) *value = v >= 2 ? stream_fns(v - 2).NP : 0;
     else if (!strcmp(name, "in_flight")) *value = v >= 2 ? stream_fns(v - 2).U : 4;
-    else if (!strcmp(name, "ring_slots")) *value = v >= 2 ? h->slots : 0;
-    else if (!strcmp(name, "slot_bytes")) *value = v >= 2 ? h->slot_bytes : 0;
+    else if (!strcmp(name, "ring_slots")) *value = v >= 2 ? g.slots : 0;
+    else if (!strcmp(name, "pinned_tiles")) *value = v >= 2 ? g.pinned : 0;
+    else if (!strcmp(name, "slot_bytes")) *value = v >= 2 ? g.slot_bytes : 0;
     else if (!strcmp(name, "resident_rows")) *value = resident_rows(h, v);
+    else if (!strcmp(name, "fold")) *value = fold_effective(h, v, 0, g) ? 1 : 0;
+    else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
+    else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
+    else if (!strcmp(name, "from_hbm")) *value = g.from_hbm ? 1 : 0;
     else return CG_EINVAL;
     return CG_OK;
 }
@@ -647,15 +869,16 @@ extern "C" int cg_probe_read_bandwidth(cg_handle* h, const void* d_buf, size_t b
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
-    CK(cudaEventCreate(&e1));
+    cudaError_t e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); CK(e); }
     const size_t n16 = bytes / 16;
     unsigned* sink = reinterpret_cast<unsigned*>(&h->scal->dot_out);
     const uint4* buf = static_cast<const uint4*>(d_buf);
     k_probe_read<<<h->sms * 4, 512, 0, st>>>(buf, n16, sink);          // warm-up (and L2 fill)
-    cudaEventRecord(e0, st);
+    e = cudaEventRecord(e0, st);
     for (int r = 0; r < reps; ++r) k_probe_read<<<h->sms * 4, 512, 0, st>>>(buf, n16, sink);
-    cudaEventRecord(e1, st);
-    cudaError_t e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventRecord(e1, st);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
     float ms = 0.f;
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
@@ -681,15 +904,16 @@ extern "C" int cg_check_csr(cg_handle* h, void* cuda_stream) {
 extern "C" int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_stream) {
     if (!h || !d_x || !d_y || d_x == d_y || !aligned16(d_x) || !aligned16(d_y)) return CG_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int v = pick_variant(h);
+    Geo g;
+    const int v = pick_variant(h, &g);
     Params P;
-    fill_params(h, &P, nullptr, nullptr, 0.0, 0, nullptr, 0, v);
+    fill_params(h, &P, nullptr, nullptr, 0.0, 0, nullptr, 0, v, g);
     if (v == 1) {
         k_spmv<<<h->grid_generic, kThreads, 0, st>>>(P, d_x, d_y);
     } else {
         const StreamFns& f = stream_fns(v - 2);
         void* args[] = {&P, &d_x, &d_y};
-        CK(cudaLaunchKernel(f.spmv, dim3(h->sms), dim3(32 * (f.W + f.NP)), args, stream_smem(h), st));
+        CK(cudaLaunchKernel(f.spmv[g.cmp], dim3(h->sms), dim3(32 * (f.W + f.NP)), args, g.smem, st));
     }
     CK(cudaGetLastError());
     h->launches = 1;
@@ -714,7 +938,7 @@ extern "C" int cg_dot(cg_handle* h, const double* d_a, const double* d_b, double
 
 // K1, K2, K3 of `iters` iterations as separate launches (captured into the graph of loop
 // mode 1, issued directly in loop mode 2).
-static int launch_iteration_kernels(cg_handle* h, int v, cudaStream_t st, int iters) {
+static int launch_iteration_kernels(cg_handle* h, int v, const Geo& g, cudaStream_t st, int iters) {
     const int G = variant_grid(h, v);
     for (int it = 0; it < iters; ++it) {
         int s = it & 1;
@@ -725,42 +949,44 @@ static int launch_iteration_kernels(cg_handle* h, int v, cudaStream_t st, int it
         } else {
             const StreamFns& f = stream_fns(v - 2);
             const dim3 blk(32 * (f.W + f.NP));
-            const size_t smem = stream_smem(h);
             void* args[] = {&h->dparams, &s};
-            CK(cudaLaunchKernel(f.k1, dim3(G), blk, args, smem, st));
-            CK(cudaLaunchKernel(f.k2, dim3(G), blk, args, smem, st));
-            CK(cudaLaunchKernel(f.k3, dim3(G), blk, args, smem, st));
+            CK(cudaLaunchKernel(f.k1[g.cmp], dim3(G), blk, args, g.smem, st));
+            CK(cudaLaunchKernel(f.k2, dim3(G), blk, args, g.smem, st));
+            CK(cudaLaunchKernel(f.k3, dim3(G), blk, args, g.smem, st));
         }
     }
     CK(cudaGetLastError());
     return CG_OK;
 }
 
-static int ensure_graph(cg_handle* h, int v) {
+static int ensure_graph(cg_handle* h, int v, const Geo& g) {
     const int G = variant_grid(h, v);
-    if (h->gexec && h->gexec_variant == v && h->gexec_chunk == h->chunk && h->gexec_grid == G)
+    if (h->gexec && h->gexec_variant == v && h->gexec_chunk == h->chunk && h->gexec_grid == G &&
+        h->gexec_cmp == g.cmp && h->gexec_smem == g.smem)
         return CG_OK;
     if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
-    cudaGraph_t g = nullptr;
+    cudaGraph_t gr = nullptr;
     if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    int rc = launch_iteration_kernels(h, v, h->cap_stream, h->chunk);
-    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
-    if (rc != CG_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    int rc = launch_iteration_kernels(h, v, g, h->cap_stream, h->chunk);
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &gr);
+    if (rc != CG_OK) { if (gr) cudaGraphDestroy(gr); return rc; }
     CK(e);
-    e = cudaGraphInstantiate(&h->gexec, g, 0);
-    cudaGraphDestroy(g);
+    e = cudaGraphInstantiate(&h->gexec, gr, 0);
+    cudaGraphDestroy(gr);
     CK(e);
-    h->gexec_variant = v; h->gexec_chunk = h->chunk; h->gexec_grid = G;
+    h->gexec_variant = v; h->gexec_chunk = h->chunk; h->gexec_grid = G; h->gexec_cmp = g.cmp; h->gexec_smem = g.smem;
     return CG_OK;
 }
 
-static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, double rtol, long long maxit,
+static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol, long long maxit,
                       double* d_hist, int precond, int64_t* h_iters, double* h_res, cudaStream_t st) {
+    Geo g;
+    const int v = pick_variant(h, &g);
     const int G = variant_grid(h, v);
     h->launches = 0;
     if (precond && !h->dinv_ready) {
-        Params P; fill_params(h, &P, d_b, d_x, rtol, maxit, d_hist, precond, v);
+        Params P; fill_params(h, &P, d_b, d_x, rtol, maxit, d_hist, precond, v, g);
         CK(cudaMemsetAsync(&h->scal->diag_bad, 0, sizeof(int), st));
         k_diag_inv<<<h->sms * 4, 256, 0, st>>>(P);
         CK(cudaGetLastError());
@@ -769,7 +995,7 @@ static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, doubl
     }
     // zero the iteration state (everything before `check`), keep check / statistics
     CK(cudaMemsetAsync(h->scal, 0, offsetof(Scal, check), st));
-    fill_params(h, h->h_params, d_b, d_x, rtol, maxit, d_hist, precond, v);
+    fill_params(h, h->h_params, d_b, d_x, rtol, maxit, d_hist, precond, v, g);
 
     if (h->loop == 0) {
         Params P = *h->h_params;
@@ -779,16 +1005,19 @@ static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, doubl
         } else {
             const StreamFns& f = stream_fns(v - 2);
             const int R = resident_rows(h, v);
-            const int ri = R == 2 ? 1 : R == 4 ? 2 : 0;
-            h->last_resident = R;
+            const bool fold = fold_effective(h, v, precond, g);
+            const int kind = R == 0 ? (precond ? kR0Jacobi : kR0)
+                           : R == 2 ? (precond ? kR2Jacobi : fold ? kR2Fold : kR2)
+                                    : (precond ? kR4Jacobi : fold ? kR4Fold : kR4);
+            h->last_resident = R; h->last_fold = fold ? 1 : 0;
             CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));        // arm the all-reduce slots
-            CK(cudaLaunchCooperativeKernel(f.persistent[ri][precond ? 1 : 0], dim3(G), dim3(32 * (f.W + f.NP)),
-                                           args, stream_smem(h), st));
+            CK(cudaLaunchCooperativeKernel(f.persistent[g.cmp][kind], dim3(G), dim3(32 * (f.W + f.NP)),
+                                           args, g.smem, st));
         }
         h->launches += 1;
     } else {
         CK(cudaMemcpyAsync(h->dparams, h->h_params, sizeof(Params), cudaMemcpyHostToDevice, st));
-        if (h->loop == 1) { int rc = ensure_graph(h, v); if (rc != CG_OK) return rc; }
+        if (h->loop == 1) { int rc = ensure_graph(h, v, g); if (rc != CG_OK) return rc; }
         if (v == 1) {
             k_init_spmv<<<G, kThreads, 0, st>>>(h->dparams);
             k_init_residual<<<G, kThreads, 0, st>>>(h->dparams);
@@ -796,20 +1025,19 @@ static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, doubl
         } else {
             const StreamFns& f = stream_fns(v - 2);
             const dim3 blk(32 * (f.W + f.NP));
-            const size_t smem = stream_smem(h);
             void* args[] = {&h->dparams};
-            CK(cudaLaunchKernel(f.init_spmv, dim3(G), blk, args, smem, st));
-            CK(cudaLaunchKernel(f.init_residual, dim3(G), blk, args, smem, st));
-            CK(cudaLaunchKernel(f.init_scalars, dim3(G), blk, args, smem, st));
+            CK(cudaLaunchKernel(f.init_spmv[g.cmp], dim3(G), blk, args, g.smem, st));
+            CK(cudaLaunchKernel(f.init_residual, dim3(G), blk, args, g.smem, st));
+            CK(cudaLaunchKernel(f.init_scalars, dim3(G), blk, args, g.smem, st));
         }
         CK(cudaGetLastError());
         h->launches += 3;
         while (true) {
             CK(cudaMemcpyAsync(h->h_scal, h->scal, sizeof(Scal), cudaMemcpyDeviceToHost, st));
             CK(cudaStreamSynchronize(st));
-            if (h->h_scal->st[0].stop) break;
+            if (h->h_scal->st[0].stop || h->h_scal->abort) break;
             if (h->loop == 1) { CK(cudaGraphLaunch(h->gexec, st)); }
-            else { int rc = launch_iteration_kernels(h, v, st, h->chunk); if (rc != CG_OK) return rc; }
+            else { int rc = launch_iteration_kernels(h, v, g, st, h->chunk); if (rc != CG_OK) return rc; }
             h->launches += 3LL * h->chunk;
         }
     }
@@ -817,6 +1045,7 @@ static int solve_impl(cg_handle* h, int v, const double* d_b, double* d_x, doubl
     CK(cudaStreamSynchronize(st));
     if (h_iters) *h_iters = h->h_scal->out_iters;
     if (h_res) *h_res = h->h_scal->out_res;
+    if (h->h_scal->abort || h->h_scal->out_status == CG_ETIMEOUT) return CG_ETIMEOUT;
     return (int)h->h_scal->out_status;
 }
 
@@ -825,7 +1054,7 @@ static int solve_checked(cg_handle* h, const double* d_b, double* d_x, double rt
     if (!h || !d_b || !d_x || d_b == d_x) return CG_EINVAL;
     if (!(rtol >= 0.0) || maxit < 0) return CG_EINVAL;          // also rejects NaN
     if (!aligned16(d_b) || !aligned16(d_x) || (reinterpret_cast<uintptr_t>(d_hist) & 7u)) return CG_EINVAL;
-    return solve_impl(h, pick_variant(h), d_b, d_x, rtol, maxit, d_hist, precond, h_iters, h_res,
+    return solve_impl(h, d_b, d_x, rtol, maxit, d_hist, precond, h_iters, h_res,
                       static_cast<cudaStream_t>(stream));
 }
 

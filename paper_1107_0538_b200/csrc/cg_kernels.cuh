@@ -43,6 +43,8 @@ struct Scal {             // device-resident scalar state, zeroed before each so
     double thresh;        // rtol * ||b||
     int brk[2];           // breakdown seen by K2 of this parity
     unsigned long long bar;       // grid barrier arrival counter
+    int abort;            // a device-side spin ran out of its budget (watchdog): the results are void
+    int pad0;
     long long out_iters;  // result block, copied to the host at the end
     long long out_status;
     double out_res;
@@ -51,6 +53,8 @@ struct Scal {             // device-resident scalar state, zeroed before each so
     int diag_bad;         // Jacobi: a diagonal entry is missing or not positive
     int max_row_len;      // cg_create statistics
     int max_tile_nnz;
+    int idx_count;        // cg_compress_index: distinct column offsets found
+    int idx_overflow;     //                    more than kMaxCodes of them (or the hash table filled up)
 };
 
 struct Params {
@@ -85,11 +89,17 @@ struct Params {
     int pinned;           // P: tiles per CTA that stay in their slot for the whole solve
     int stream_slots;     // Q: slots the other tiles stream through (a multiple of the producer count)
     int slot_bytes;       // cap * 12 + 144, rounded up to 128
-    double* p2;           // second p buffer of the folded loop (cg_stream_kernels.cuh)
-    int fold;             // 1: fold K3 into the next K1's gathers (two grid syncs per iteration)
+    double2* pr0;         // the two {p, r} pair buffers of the folded loop (cg_stream_kernels.cuh)
+    double2* pr1;
     int lookahead;        // producer run-ahead (tiles) into a pass the consumers have not started
-    int l2_prefetch;      // 1: producers prefetch tiles into the L2 a batch ahead (only with l2_stream)
     int l2_stream;        // 1: the matrix does not fit the L2 -> evict-first hint on its copies
+    // compressed index (cg_compress_index): one record per tile, see cg_stream.cuh
+    int cmp;              // 1: slots hold {vals span, index record}
+    int rec_stride;       // bytes per record: 80 + 32 * (longest row), a multiple of 16
+    const unsigned char* idx_rec;   // records, tile t at idx_rec + t * rec_stride
+    const int* idx_off;   // kMaxCodes column offsets (col - row) named by the codes
+    long long spin_budget;          // cycles any device-side spin may last before the watchdog trips
+    int inject_fault;     // tests: producer warp 0 of CTA 0 never copies its inject_fault-th tile (0 = off)
 };
 
 constexpr int kTraceSlots = 16;  // stamps per iteration and CTA, see k_persistent
@@ -107,7 +117,10 @@ __device__ __forceinline__ int ld_stream_s32(const int* p) {
     return v;
 }
 __device__ __forceinline__ double ld_global_f64(const double* p) {
-    double v;   // explicit global-space load (vectors are read AND written inside one launch: no .nc)
+    double v;   // explicit global-space load (vectors are read AND written inside one launch: no .nc).
+    // No "memory" clobber (it would serialise the batched gathers against the shared-memory
+    // loads around them): a thread that reads back its OWN earlier plain store through this
+    // must put a compiler barrier between the two (the one place is the R = 0 prologue).
     asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
@@ -155,18 +168,29 @@ __device__ __forceinline__ double sum_partials(const double* part, int G, double
 }
 
 // Grid-wide barrier for the cooperative persistent kernel (all CTAs co-resident).
-// One arrival counter, never reset inside a solve; `epoch` is the local target.
-__device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned int G,
-                                             unsigned long long& epoch) {
+// One arrival counter, never reset inside a solve; `epoch` is the local target.  The spin is
+// bounded: after `budget` cycles thread 0 raises *abort and the barrier returns true (in every
+// thread of the CTA), after which the caller leaves the loop.
+__device__ __forceinline__ bool grid_barrier(unsigned long long* bar, unsigned int G,
+                                             unsigned long long& epoch, long long budget, int* abort) {
     __syncthreads();
+    int dead = 0;
     if (threadIdx.x == 0) {
         epoch += G;
         __threadfence();
         red_release_add_u64(bar, 1ULL);
-        while (ld_acquire_u64(bar) < epoch) { }
+        const long long t0 = clock64();
+        unsigned n = 0;
+        while (ld_acquire_u64(bar) < epoch) {
+            if ((++n & 0x3ffu) == 0u && clock64() - t0 > budget) {
+                *reinterpret_cast<volatile int*>(abort) = 1;
+                dead = 1;
+                break;
+            }
+        }
         __threadfence();                   // also invalidates this SM's L1 (CCTL.IVALL)
     }
-    __syncthreads();
+    return __syncthreads_or(dead) != 0;
 }
 
 // ---------------------------------------------------------------- K1, variant A

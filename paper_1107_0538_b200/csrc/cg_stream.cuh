@@ -15,20 +15,30 @@
 // floating-point operations in the same order and gives bitwise identical results.
 //
 // K1 data flow.  NP extra warps (the producers) walk the CTA's tiles in order and,
-// for each, wait for a free ring slot and issue three cp.async.bulk copies (SASS UBLKCP)
-// into it: the tile's contiguous vals span, its colind span and its 33 row pointers (36
-// ints from a padded copy of rowptr).  Consumers wait on the slot's "full" mbarrier, copy
-// their row bounds and entries from shared memory into registers, hand the slot back, then
-// gather x through L1/L2.  No consumer ever waits on a row-pointer or matrix load from
-// global memory; the only global loads in its loop are the x gathers.  In the persistent
-// kernel the producers run ahead into the next iteration's tiles (the matrix does not
-// change) while the consumers do K2/K3 and wait at the grid barriers, so K1 starts on a
-// full ring.
+// for each, wait for a free ring slot and issue cp.async.bulk copies (SASS UBLKCP) into it.
+// Two slot formats (template flag CMP):
+//   plain CSR     the tile's contiguous vals span, its colind span and its 33 row pointers (36
+//                 ints from a padded copy of rowptr): 12 B per entry, three copies;
+//   compressed    (cg_compress_index) the vals span and ONE index record built at setup: 33
+//                 relative row starts (u16) and one byte per entry that names the entry's column
+//                 offset col - row in a table of <= 256 distinct offsets: 9 B per entry, two
+//                 copies.  Entries keep their CSR order, so both formats give the same bits.
+// Consumers wait on the slot's "full" mbarrier, copy their row bounds and entries from shared
+// memory into registers, hand the slot back, then gather x through L1/L2.  No consumer ever
+// waits on a row-pointer or matrix load from global memory; the only global loads in its loop
+// are the x gathers.  In the persistent kernel the producers run ahead into the next
+// iteration's tiles (the matrix does not change) while the consumers do K2/K3 and wait at the
+// grid barriers, so K1 starts on a full ring.
 //
 // Alignment of the bulk copies: source, destination and size must be multiples of 16
-// bytes.  A tile's span [s, e) is widened to [s & ~3, (e + 3) & ~3), clamped to nnz & ~3;
-// the <= 3 entries of the whole matrix past that bound are written into the slot by the
-// producer with ordinary loads/stores, so nothing outside the caller's arrays is touched.
+// bytes.  A tile's span [s, e) is widened to [s & ~A, (e + A) & ~A) with A = 3 (plain: colind
+// is the 4-byte array) or A = 1 (compressed: only vals come from the caller's arrays), clamped
+// to nnz & ~A; the <= A entries of the whole matrix past that bound are written into the slot
+// by the producer with ordinary loads/stores, so nothing outside the caller's arrays is touched.
+//
+// Every spin in this file is bounded (bounded_spin): after Params::spin_budget cycles the CTA
+// raises Scal::abort, stops waiting and leaves the solve at the next collective point; the host
+// then returns CG_ETIMEOUT instead of hanging the device.
 #pragma once
 #include "cg_kernels.cuh"
 
@@ -42,7 +52,10 @@ constexpr int kBarGrid = 160;        // max CTAs of a streamed persistent grid (
 constexpr int kBarM = kBarGrid / 32;
 constexpr int kMaxSlots = 64;
 constexpr int kSmemTail = 2304;      // mbarriers + reduction scratch + flags after the slots
-constexpr int kRedTot = 96;          // red[0..95]: per-warp partials (3 values x 32 warps); red[96..]: totals
+constexpr int kRedTot = 96;          // red[0..95]: per-warp partials (3 values x 32 warps); red[96..98]: totals; red[99]: abort
+constexpr int kRecHdr = 80;          // compressed index record: 33 u16 row starts, [33] = s & 1, padded to 80 bytes
+constexpr int kMaxCodes = 256;       // distinct column offsets a compressed index can name
+constexpr int kOffTabBytes = kMaxCodes * 4;
 
 // W consumer warps + NP producer warps per CTA; W + NP is a multiple of 4 so the warps spread
 // evenly over the SM's four sub-partitions (their register files bound the registers per thread).
@@ -52,26 +65,32 @@ template <int W, int NP> struct Shape {
     static constexpr int kConsumerThreads = 32 * W;
     static constexpr int kThreads = 32 * (W + NP);
 };
-constexpr int kSlotQuantum = 20;     // ring depths are multiples of this (lcm of the producer counts 4 and 5) when they can be
 
 struct Ring {
     unsigned char* slots;
     uint64_t* full;
     uint64_t* empty;
     double* red;                      // 104 doubles of reduction scratch (see kRedTot)
-    volatile int* ctl;                // [0] stop flag, [1] passes consumed (low), [2] (high), [3] passes started
+    volatile int* ctl;                // [0] stop flag, [1] passes consumed (low), [2] (high), [3] passes started,
+                                      // [4] a spin of this CTA ran out of budget (watchdog)
     volatile unsigned* tag;           // per slot: 1 + number (mod 2^32) of the tile last issued into it
+    const int* offtab;                // compressed index: column offset per code (shared-memory copy)
     int S, slot_bytes, cap;
     int P, Q;                         // pinned slots [0, P) and streaming slots [P, P + Q), P + Q <= S
+    long long budget;                 // cycles a spin may last
+    Scal* scal;
     unsigned long long* acc;          // optional: cycles this thread waited on full barriers (trace)
     __device__ __forceinline__ double* vals(int slot) const {
         return reinterpret_cast<double*>(slots + (size_t)slot * slot_bytes);
     }
-    __device__ __forceinline__ int* cols(int slot) const {
+    __device__ __forceinline__ int* cols(int slot) const {             // plain slots
         return reinterpret_cast<int*>(slots + (size_t)slot * slot_bytes + (size_t)cap * 8);
     }
     __device__ __forceinline__ int* rp(int slot) const {
         return reinterpret_cast<int*>(slots + (size_t)slot * slot_bytes + (size_t)cap * 12);
+    }
+    __device__ __forceinline__ unsigned char* rec(int slot) const {    // compressed slots
+        return slots + (size_t)slot * slot_bytes + (size_t)cap * 8;
     }
 };
 
@@ -79,6 +98,7 @@ __device__ __forceinline__ Ring ring_view(const Params& P, unsigned char* dyn) {
     Ring rg;
     rg.S = P.slots; rg.slot_bytes = P.slot_bytes; rg.cap = P.cap; rg.acc = nullptr;
     rg.P = P.pinned; rg.Q = P.stream_slots;
+    rg.budget = P.spin_budget; rg.scal = P.scal;
     rg.slots = dyn;
     unsigned char* tail = dyn + (size_t)P.slots * P.slot_bytes;
     rg.full = reinterpret_cast<uint64_t*>(tail);
@@ -86,23 +106,25 @@ __device__ __forceinline__ Ring ring_view(const Params& P, unsigned char* dyn) {
     rg.red = reinterpret_cast<double*>(rg.empty + kMaxSlots);
     rg.ctl = reinterpret_cast<volatile int*>(rg.red + 104);
     rg.tag = reinterpret_cast<volatile unsigned*>(rg.ctl + 8);       // kMaxSlots entries
+    rg.offtab = reinterpret_cast<const int*>(tail + kSmemTail);      // kOffTabBytes, only with a compressed index
     return rg;
 }
 
-// Called by every thread of the CTA (producer warp included) before anything else.
-__device__ __forceinline__ void ring_init(const Ring& rg) {
+// Called by every thread of the CTA (producer warps included) before anything else.
+__device__ __forceinline__ void ring_init(const Params& P, const Ring& rg) {
     if ((int)threadIdx.x < rg.S) {
         mbar_init(&rg.full[threadIdx.x], 1);
         mbar_init(&rg.empty[threadIdx.x], 1);
         rg.tag[threadIdx.x] = 0u;
     }
-    if (threadIdx.x == 0) { rg.ctl[0] = 0; rg.ctl[1] = 0; rg.ctl[2] = 0; rg.ctl[3] = 0; }
+    if (threadIdx.x < 8) rg.ctl[threadIdx.x] = 0;
+    if (P.cmp && threadIdx.x < kMaxCodes) const_cast<int*>(rg.offtab)[threadIdx.x] = P.idx_off[threadIdx.x];
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 }
 
-// Barrier among the consumer warps only (the producer never joins it).
+// Barrier among the consumer warps only (the producers never join it).
 template <int W> __device__ __forceinline__ void consumer_sync() {
     asm volatile("bar.sync 1, %0;" :: "n"(32 * W) : "memory");
 }
@@ -115,63 +137,76 @@ __device__ __forceinline__ void cta_tiles(const Params& P, int cta, int G, long 
     Tc = (int)(te - tb);
 }
 
+// ---------------------------------------------------------------- watchdog
+
+// Spin until pred() holds.  Gives up (returns false) once the spin has lasted rg.budget cycles
+// or another warp of this CTA has given up: it then raises the CTA's flag (ctl[4]) and the
+// solve's (Scal::abort).  The clock is read once per 1024 polls, so the happy path costs nothing.
+template <class Pred>
+__device__ __forceinline__ bool bounded_spin(const Ring& rg, Pred pred) {
+    if (pred()) return true;
+    const long long t0 = clock64();
+    for (unsigned n = 1;; ++n) {
+        if (pred()) return true;
+        if ((n & 0x3ffu) == 0u && (rg.ctl[4] != 0 || clock64() - t0 > rg.budget)) {
+            rg.ctl[4] = 1;
+            *reinterpret_cast<volatile int*>(&rg.scal->abort) = 1;
+            return false;
+        }
+    }
+}
+__device__ __forceinline__ bool mbar_wait_bounded(const Ring& rg, uint64_t* bar, uint32_t parity) {
+    return bounded_spin(rg, [&] { return mbar_try_wait(bar, parity); });
+}
+
 // ---------------------------------------------------------------- producer
 
+template <bool CMP>
 __device__ __forceinline__ void producer_issue(const Params& P, const Ring& rg, int slot, long long t,
-                                               int s, int e, uint64_t policy, unsigned tag) {
-    const int s4 = s & ~3;
-    const int lim = (int)(P.nnz & ~3LL);              // last entry reachable by bulk copies
-    int e4 = (e + 3) & ~3;
+                                               int s, int e, uint64_t policy, unsigned tag, bool drop) {
+    constexpr int A = CMP ? 1 : 3;                     // span alignment in entries (16 bytes of the narrowest array)
+    const int s4 = s & ~A;
+    const int lim = (int)(P.nnz & ~(long long)A);     // last entry reachable by bulk copies
+    int e4 = (e + A) & ~A;
     if (e4 > lim) e4 = lim;
-    const int cnt = e4 > s4 ? e4 - s4 : 0;            // multiple of 4
+    const int cnt = e4 > s4 ? e4 - s4 : 0;            // multiple of A + 1
     double* sv = rg.vals(slot);
-    int* sc = rg.cols(slot);
-    if (e > lim) {                                    // the matrix's last <= 3 entries, by hand
+    if (e > lim) {                                    // the matrix's last <= A entries, by hand
         for (int k = (lim > s4 ? lim : s4); k < e; ++k) {
             sv[k - s4] = ld_stream_f64(P.vals + k);
-            sc[k - s4] = ld_stream_s32(P.colind + k);
+            if (!CMP) rg.cols(slot)[k - s4] = ld_stream_s32(P.colind + k);
         }
     }
     uint64_t* bar = &rg.full[slot];
     rg.tag[slot] = tag;                               // before the arrive below (release): see consume_tile
-    mbar_expect_tx(bar, (uint32_t)cnt * 12u + (uint32_t)kRpInts * 4u);
+    const uint32_t meta = CMP ? (uint32_t)P.rec_stride : (uint32_t)kRpInts * 4u;
+    mbar_expect_tx(bar, (uint32_t)cnt * (CMP ? 8u : 12u) + meta);
+    if (drop) return;                                 // fault injection (option "inject_fault"): the copies never come
     if (cnt > 0) {
         if (P.l2_stream) {
             bulk_g2s(sv, P.vals + s4, (uint32_t)cnt * 8u, bar, policy);
-            bulk_g2s(sc, P.colind + s4, (uint32_t)cnt * 4u, bar, policy);
+            if (!CMP) bulk_g2s(rg.cols(slot), P.colind + s4, (uint32_t)cnt * 4u, bar, policy);
         } else {
             bulk_g2s_plain(sv, P.vals + s4, (uint32_t)cnt * 8u, bar);
-            bulk_g2s_plain(sc, P.colind + s4, (uint32_t)cnt * 4u, bar);
+            if (!CMP) bulk_g2s_plain(rg.cols(slot), P.colind + s4, (uint32_t)cnt * 4u, bar);
         }
     }
-    bulk_g2s_plain(rg.rp(slot), P.rp_pad + t * kTileRows, (uint32_t)kRpInts * 4u, bar);
-}
-
-constexpr int kPrefetchBatch = 8;    // tiles per producer warp sent towards the L2 ahead of their ring copies
-
-// Start a tile's vals / colind spans towards the L2 (same widening and clamping as producer_issue).
-__device__ __forceinline__ void prefetch_tile_l2(const Params& P, int s, int e) {
-    const int s4 = s & ~3;
-    const int lim = (int)(P.nnz & ~3LL);
-    int e4 = (e + 3) & ~3;
-    if (e4 > lim) e4 = lim;
-    const int cnt = e4 > s4 ? e4 - s4 : 0;
-    if (cnt > 0) {
-        const uint64_t pol = l2_policy_evict_first();      // must not push p out of the L2
-        asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;"
-                     :: "l"(P.vals + s4), "r"((uint32_t)cnt * 8u), "l"(pol) : "memory");
-        asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;"
-                     :: "l"(P.colind + s4), "r"((uint32_t)cnt * 4u), "l"(pol) : "memory");
+    if (CMP) {
+        const unsigned char* src = P.idx_rec + (size_t)t * (size_t)P.rec_stride;
+        if (P.l2_stream) bulk_g2s(rg.rec(slot), src, meta, bar, policy);
+        else             bulk_g2s_plain(rg.rec(slot), src, meta, bar);
+    } else {
+        bulk_g2s_plain(rg.rp(slot), P.rp_pad + t * kTileRows, meta, bar);
     }
 }
 
-// Pinned and streamed tiles.  When the matrix is L2-resident anyway (it is re-read every
-// iteration), the first P tiles of a CTA are PINNED: tile j < P is copied into slot j once,
-// in the first pass, and stays there for the whole solve (no L2 traffic, no shared-memory
-// write, no producer work for it in later iterations).  The other Ts = Tc - P tiles of a
-// pass are STREAMED through the Q slots [P, P + Q): streamed tile number seq (counted over
-// all passes) uses slot P + seq mod Q.  P = Tc (everything pinned, nothing streamed) when
-// the CTA's whole slice fits the ring.
+// Pinned and streamed tiles.  The first P tiles of a CTA are PINNED: tile j < P is copied into
+// slot j once, in the first pass, and stays there for the whole solve (no L2 traffic, no
+// shared-memory write, no producer work for it in later iterations).  The other Ts = Tc - P
+// tiles of a pass are STREAMED through the Q slots [P, P + Q): streamed tile number seq
+// (counted over all passes) uses slot P + seq mod Q.  The host pins everything (P >= Tc) when
+// the CTA's whole slice fits the ring and nothing otherwise; a mixed split (option "pin" >= 2)
+// exists for tests and measurements.
 //
 // A pass starts at stream position `pos` = (slot offset, parity, number) of its first streamed
 // tile; streamed tile i of the pass sits i slots further on.
@@ -199,7 +234,9 @@ __device__ __forceinline__ RingPos ring_next_pass(const Ring& rg, RingPos p, int
 // time, one per lane; a CTA with <= 32 tiles fetches them once.  The warp runs ahead of the
 // consumers by as many tiles as the ring has free slots, also into the next pass, but there
 // by at most P.lookahead tiles until the consumers start that pass (ctl[3] counts the
-// passes they have started).
+// passes they have started).  Its waits end through the stop flag (ctl[0], raised by the
+// consumers at the end of a persistent solve) or the CTA's watchdog flag (ctl[4]).
+template <bool CMP>
 __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, long long tb, int Tc,
                                               long long passes, int q, int NP) {
     const int lane = threadIdx.x & 31;
@@ -208,6 +245,9 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     const int Pn = rg.P < Tc ? rg.P : Tc;                  // my CTA's pinned tiles: [0, Pn)
     const int Ts = Tc - Pn;                                 // streamed tiles per pass
     const int Q = rg.Q;
+    // fault injection (tests): producer warp 0 of CTA 0 announces its `inject_fault`-th tile and never copies it
+    const int fault_at = (P.inject_fault > 0 && blockIdx.x == 0 && q == 0) ? P.inject_fault : 0;
+    int issued = 0;
     int s = 0, e = 0;
     const bool cached = Tc <= 32;                           // lane l keeps the bounds of tile l
     if (cached && lane < Tc) {
@@ -228,7 +268,8 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
             const int j = q + l * NP;
             const int si = __shfl_sync(0xffffffffu, cached ? s : ps, cached ? j : l);
             const int ei = __shfl_sync(0xffffffffu, cached ? e : pe, cached ? j : l);
-            if (lane == 0) producer_issue(P, rg, j, tb + j, si, ei, policy, (unsigned)j + 1u);
+            ++issued;
+            if (lane == 0) producer_issue<CMP>(P, rg, j, tb + j, si, ei, policy, (unsigned)j + 1u, issued == fault_at);
         }
     }
     if (Ts <= 0 || Q <= 0) return;
@@ -237,19 +278,11 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     int j = q;                                              // = seq - pass * Ts, index among the streamed tiles
     while (j >= Ts) { j -= Ts; ++pass; }
     unsigned slot = (unsigned)q, par = 0;                   // = seq mod Q, (seq / Q) & 1
-    // Optional (option "l2_prefetch", off by default), matrix >> L2: the producers start every
-    // tile towards the L2 one batch of their tiles before they copy it into shared memory
-    // (cp.async.bulk.prefetch.L2 needs no slot and no barrier), to have more bytes in flight
-    // towards HBM than the ring holds.  Measured at config 4: with 4 tiles per warp ahead K1
-    // drops from 451 k to 429 k cycles on average but the CTAs drift apart (the barrier
-    // after K1 grows from 16 k to 40 k cycles): no gain; 8 and 16 ahead are slower outright.
-    const bool pf = P.l2_stream != 0 && P.l2_prefetch != 0;
-    const int B = cached ? 32 : (pf ? (P.l2_prefetch > 1 ? P.l2_prefetch : kPrefetchBatch) : 32);
-    if (!cached && lane < B) {             // bounds of my first batch
+    constexpr int B = 32;                                   // tile bounds are fetched 32 at a time, one per lane
+    if (!cached) {                                          // bounds of my first batch
         const int jl = (int)(((long long)j + (long long)lane * NP) % Ts);
         s = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows);
         e = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows + kTileRows);
-        if (pf) prefetch_tile_l2(P, s, e);
     }
     bool stopped = false;
     unsigned long long t_wait = 0;
@@ -257,23 +290,20 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
     const bool timing = P.trace != nullptr;
     while (pass < passes && !stopped) {
         int s2 = 0, e2 = 0;
-        if (!cached) {                     // bounds of the batch AFTER this one; start them towards the L2
+        if (!cached) {                     // bounds of the batch AFTER this one
             const int jl = (int)(((long long)j + (long long)(B + lane) * NP) % Ts);
-            if (lane < B) {
-                s2 = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows);
-                e2 = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows + kTileRows);
-                if (pf) prefetch_tile_l2(P, s2, e2);
-            }
+            s2 = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows);
+            e2 = ld_stream_s32(P.rp_pad + (tb + Pn + jl) * kTileRows + kTileRows);
         }
         for (int l = 0; l < B && pass < passes; ++l) {
             int ok = 1;
             if (lane == 0) {
                 const long long t0 = timing ? clock64() : 0;
                 if (passes > 1 && j >= P.lookahead) {
-                    while ((long long)rg.ctl[3] <= pass) { if (rg.ctl[0]) { ok = 0; break; } }
+                    while ((long long)rg.ctl[3] <= pass) { if (rg.ctl[0] | rg.ctl[4]) { ok = 0; break; } }
                 }
                 while (ok && !mbar_try_wait(&rg.empty[Pn + slot], par ^ 1u)) {
-                    if (rg.ctl[0]) ok = 0;
+                    if (rg.ctl[0] | rg.ctl[4]) ok = 0;
                 }
                 if (timing) t_wait += (unsigned long long)(clock64() - t0);
             }
@@ -282,7 +312,9 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
             const int src = cached ? Pn + j : l;
             const int si = __shfl_sync(0xffffffffu, s, src);
             const int ei = __shfl_sync(0xffffffffu, e, src);
-            if (lane == 0) producer_issue(P, rg, Pn + (int)slot, tb + Pn + j, si, ei, policy, (unsigned)seq + 1u);
+            ++issued;
+            if (lane == 0) producer_issue<CMP>(P, rg, Pn + (int)slot, tb + Pn + j, si, ei, policy, (unsigned)seq + 1u,
+                                               issued == fault_at);
             seq += (unsigned long long)NP;
             j += NP;
             while (j >= Ts) { j -= Ts; ++pass; }
@@ -295,7 +327,7 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
         unsigned long long* row = P.trace + ((size_t)blockIdx.x * (P.trace_iters + 1) + P.trace_iters) * kTraceSlots;
         row[0] = t_wait; row[1] = (unsigned long long)(clock64() - t_begin); row[2] = seq / (unsigned)NP;
     }
-    if (stopped) {
+    if (stopped && rg.ctl[4] == 0) {
         // Drain: my copies for tiles nobody will consume must land before the CTA exits.  The
         // consumers finished `done` whole passes, i.e. the streamed tiles below done * Ts.
         const unsigned long long done = (((unsigned long long)(unsigned)rg.ctl[2] << 32) | (unsigned)rg.ctl[1])
@@ -303,7 +335,7 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
         unsigned long long w = done + (((unsigned long long)q + (unsigned long long)NP
                                         - done % (unsigned long long)NP) % (unsigned long long)NP);
         for (; w < seq; w += (unsigned long long)NP)
-            mbar_wait(&rg.full[Pn + (int)(w % (unsigned)Q)], (uint32_t)((w / (unsigned)Q) & 1ULL));
+            if (!mbar_wait_bounded(rg, &rg.full[Pn + (int)(w % (unsigned)Q)], (uint32_t)((w / (unsigned)Q) & 1ULL))) break;
     }
 }
 
@@ -321,6 +353,12 @@ __device__ __forceinline__ void consumers_stop(const Ring& rg, unsigned long lon
 
 // ---------------------------------------------------------------- consumer
 
+__device__ __forceinline__ double2 ld_global_f64x2(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+
 // One tile: wait for its slot, y_row = sum_k a_k x[col_k] for this lane's row.  U entries are
 // in flight per lane and trip: their column indices and values are read from shared memory,
 // then the U gathers are issued, then the FMAs go into three independent accumulators
@@ -330,13 +368,18 @@ __device__ __forceinline__ void consumers_stop(const Ring& rg, unsigned long lon
 // length a slot is held for a few hundred cycles only and nearly the whole ring is in
 // flight.  Padding entries (k >= ke) use value 0 and column 0.
 //
+// CMP: the slot holds the compressed index record: row bounds are u16 relative to the tile,
+// entry t of lane l has its code at byte [t * 32 + l] (transposed at setup: conflict-free
+// loads) and its column is row + offtab[code].
+//
 // FOLD: the gathered operand is not stored anywhere yet: it is p_new[c] = fma(beta, p_old[c],
 // r[c]), the very expression K3 evaluates for row c, recomputed here by every thread that
-// needs it (x = p_old, r = the residual K2 just stored).  Same operation, same operands, same
-// bits as the owner's own update; it saves the third grid synchronisation of an iteration.
-template <int U, bool FOLD = false>
+// needs it from the pair {p_old[c], r[c]} (one 16-byte gather; K2 stored r there).  Same
+// operation, same operands, same bits as the owner's own update; it saves the third grid
+// synchronisation of an iteration.  `x` then points at the double2 pairs.
+template <int U, bool FOLD, bool CMP, bool GF>
 __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, RingPos pos, int j,
-                                               int lane, const double* r = nullptr, double beta = 0.0) {
+                                               int lane, int row, double beta = 0.0) {
     static_assert(U % 3 == 0, "three accumulators");
     const bool pinned = j < rg.P;
     RingPos at;
@@ -347,19 +390,30 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
     // has not landed yet" (two phases apart).  The previous tile belongs to another warp, and
     // bulk copies complete out of order, so first wait until this tile has been issued into
     // the slot: from then on the barrier's pending phase is this tile's.
-    while (rg.tag[slot] != at.seq + 1u) { }
+    bool ok = bounded_spin(rg, [&] { return rg.tag[slot] == at.seq + 1u; });
     if (rg.acc) {
         const long long t0 = clock64();
-        mbar_wait(&rg.full[slot], at.par);
+        ok = ok && mbar_wait_bounded(rg, &rg.full[slot], at.par);
         *rg.acc += (unsigned long long)(clock64() - t0);
     } else {
-        mbar_wait(&rg.full[slot], at.par);
+        ok = ok && mbar_wait_bounded(rg, &rg.full[slot], at.par);
     }
-    const int* rp = rg.rp(slot);
-    const int base = rp[0] & ~3;
-    const int ks = rp[lane] - base, ke = rp[lane + 1] - base;
+    if (!__all_sync(0xffffffffu, ok)) return 0.0;      // watchdog: the slot's contents are not to be trusted
+    int ks, ke;
     const double* sv = rg.vals(slot);
-    const int* sc = rg.cols(slot);
+    const int* sc = nullptr;
+    const unsigned char* sb = nullptr;
+    if constexpr (CMP) {
+        const unsigned short* hd = reinterpret_cast<const unsigned short*>(rg.rec(slot));
+        ks = hd[lane]; ke = hd[lane + 1];
+        sv += hd[33];                                  // the vals span starts at s & ~1
+        sb = rg.rec(slot) + kRecHdr + lane;
+    } else {
+        const int* rp = rg.rp(slot);
+        const int base = rp[0] & ~3;
+        ks = rp[lane] - base; ke = rp[lane + 1] - base;
+        sc = rg.cols(slot);
+    }
     const int trips = __reduce_max_sync(0xffffffffu, (ke - ks + U - 1) / U);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
     if (trips == 0 && !pinned) {
@@ -369,37 +423,74 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
     for (int t = 0; t < trips; ++t) {
         const int k = ks + t * U;
         int c[U];
-        double v[U], xv[U];
+        double v[GF ? 1 : U], xv[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const bool ok = k + u < ke;
-            const int kk = ok ? k + u : 0;
-            const int cc = sc[kk];
-            const double vv = sv[kk];
-            c[u] = ok ? cc : 0;
-            v[u] = ok ? vv : 0.0;
+            const bool in = k + u < ke;
+            const int kk = in ? k + u : 0;
+            int cc;
+            if constexpr (CMP) cc = row + rg.offtab[sb[in ? (t * U + u) * 32 : 0]];
+            else               cc = sc[kk];
+            c[u] = in ? cc : 0;
+            if constexpr (!GF) { const double vv = sv[kk]; v[u] = in ? vv : 0.0; }
         }
-        if (t == trips - 1 && !pinned) {
+        if (!GF && t == trips - 1 && !pinned) {
             __syncwarp();                  // every lane has its last entries in registers
             if (lane == 0) mbar_arrive(&rg.empty[slot]);
         }
-#pragma unroll
-        for (int u = 0; u < U; ++u) xv[u] = ld_global_f64(x + c[u]);
         if constexpr (FOLD) {
-            double rg_[U];
+            const double2* xp = reinterpret_cast<const double2*>(x);
+            double2 pr[U];
 #pragma unroll
-            for (int u = 0; u < U; ++u) rg_[u] = ld_global_f64(r + c[u]);
+            for (int u = 0; u < U; ++u) pr[u] = ld_global_f64x2(xp + c[u]);
 #pragma unroll
-            for (int u = 0; u < U; ++u) xv[u] = fma(beta, xv[u], rg_[u]);
+            for (int u = 0; u < U; ++u) xv[u] = fma(beta, pr[u].x, pr[u].y);
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) xv[u] = ld_global_f64(x + c[u]);
         }
+        if constexpr (GF) {
+            // gather-first: the values are read from the slot while the gathers are in flight,
+            // which keeps U of them in flight with U + few registers; the slot is held meanwhile
 #pragma unroll
-        for (int u = 0; u < U; u += 3) {
-            a0 = fma(v[u], xv[u], a0);
-            a1 = fma(v[u + 1], xv[u + 1], a1);
-            a2 = fma(v[u + 2], xv[u + 2], a2);
+            for (int u = 0; u < U; u += 3) {
+                const double v0 = k + u < ke ? sv[k + u] : 0.0;
+                const double v1 = k + u + 1 < ke ? sv[k + u + 1] : 0.0;
+                const double v2 = k + u + 2 < ke ? sv[k + u + 2] : 0.0;
+                a0 = fma(v0, xv[u], a0);
+                a1 = fma(v1, xv[u + 1], a1);
+                a2 = fma(v2, xv[u + 2], a2);
+            }
+            if (t == trips - 1 && !pinned) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&rg.empty[slot]);
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; u += 3) {
+                a0 = fma(v[u], xv[u], a0);
+                a1 = fma(v[u + 1], xv[u + 1], a1);
+                a2 = fma(v[u + 2], xv[u + 2], a2);
+            }
         }
     }
     return (a0 + a1) + a2;
+}
+
+// Shapes without producer warps (NP = 0; only when every tile is pinned): consumer warp w copies
+// its own tiles w, w + W, ... into their slots, once per kernel.
+template <int W, bool CMP>
+__device__ __forceinline__ void consumers_pin_tiles(const Params& P, const Ring& rg, long long tb, int Tc) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane != 0) return;
+    const int Pn = rg.P < Tc ? rg.P : Tc;
+    const uint64_t policy = l2_policy_evict_first();
+    for (int j = warp; j < Pn; j += W) {
+        const int s = ld_stream_s32(P.rp_pad + (tb + j) * kTileRows);
+        const int e = ld_stream_s32(P.rp_pad + (tb + j) * kTileRows + kTileRows);
+        producer_issue<CMP>(P, rg, j, tb + j, s, e, policy, (unsigned)j + 1u,
+                            P.inject_fault > 0 && blockIdx.x == 0 && j == P.inject_fault - 1);
+    }
 }
 
 // ---------------------------------------------------------------- reductions
@@ -449,13 +540,17 @@ __device__ __forceinline__ double sum_partials_w(const double* part, int G, doub
 // Slot recycling: after its poll a CTA rewrites the slots it just read with the idle
 // pattern (all-ones: a NaN no arithmetic produces, published NaNs are canonicalised, and
 // cudaMemset(0xFF) arms the inboxes).  Source j writes that buffer again three all-reduces
-// later.  FENCED all-reduces (the prologue's; with the fold, the one after K2 that publishes
-// r and p) carry a gpu-scope fence before the push (release of everything the CTA wrote)
-// and one after the reset (acquire; it also invalidates this SM's L1).  The others carry
-// only their payload.  Between an all-reduce and the third one after it there is always
-// either a fenced one or the counter barrier after K3 (grid_barrier_counter, fenced on both
-// sides in every CTA), which is what orders a reset before the next write into the slot:
+// later.  FENCED all-reduces carry a gpu-scope fence before the push (release of everything
+// the CTA wrote) and one after the reset (acquire; it also invalidates this SM's L1).  The
+// others carry only their payload.  Between an all-reduce and the third one after it there
+// must be a fenced one or the counter barrier (grid_barrier_counter, fenced on both sides in
+// every CTA), which is what orders a reset before the next write into the slot:
 // reset -> my fence -> my later push or arrival -> j observes it -> j's fence -> j's write.
+// The ONE place that fixes an iteration's sequence of synchronisations, and with it this
+// invariant, is SyncPlan in cg_stream_kernels.cuh (checked there by a static_assert).
+//
+// Returns true when the watchdog tripped in this CTA (in any consumer warp before the call, or
+// in the poll): the value is the same in every consumer thread of the CTA.
 constexpr unsigned long long kIdle = 0xFFFFFFFFFFFFFFFFULL;
 constexpr int kInboxStride = 3 * kBarVals * kBarGrid;     // u64 per CTA inbox
 
@@ -472,10 +567,11 @@ __device__ __forceinline__ unsigned long long publishable(double v) {
 }
 
 template <int W, int NV, bool FENCED>
-__device__ __forceinline__ void grid_allreduce(const Params& P, double* red, unsigned& count,
+__device__ __forceinline__ bool grid_allreduce(const Params& P, const Ring& rg, unsigned& count,
                                                int cta, int G, double (&v)[NV],
                                                unsigned long long* dbg = nullptr) {
     static_assert(NV >= 1 && NV <= kBarVals && W <= 32, "slot layout");
+    double* red = rg.red;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double w[NV];
     if (dbg) dbg[0] = clock64();
@@ -508,7 +604,9 @@ __device__ __forceinline__ void grid_allreduce(const Params& P, double* red, uns
         // poll my inbox
         unsigned long long* mine = base + (size_t)cta * kInboxStride + (b * kBarVals) * kBarGrid;
         unsigned long long u[NV][kBarM];
-        bool ready;
+        bool ready, dead = false;
+        unsigned rounds = 0;
+        long long t0 = 0;
         do {
             ready = true;
 #pragma unroll
@@ -519,16 +617,26 @@ __device__ __forceinline__ void grid_allreduce(const Params& P, double* red, uns
                     u[i][m] = (j < G) ? ld_relaxed_u64(mine + i * kBarGrid + j) : 0ULL;
                     ready = ready && (u[i][m] != kIdle);
                 }
-        } while (!ready);
-        if (dbg) dbg[3] = clock64();
-        // recycle the slots just read
-#pragma unroll
-        for (int i = 0; i < NV; ++i)
-#pragma unroll
-            for (int m = 0; m < kBarM; ++m) {
-                const int j = lane + 32 * m;
-                if (j < G) st_relaxed_u64(mine + i * kBarGrid + j, kIdle);
+            if (!ready && (++rounds & 0xffu) == 0u) {          // watchdog, once per 256 poll rounds
+                if (rounds == 0x100u) t0 = clock64();
+                else if (rg.ctl[4] != 0 || clock64() - t0 > rg.budget) { dead = true; break; }
             }
+        } while (!ready);
+        dead = __any_sync(0xffffffffu, dead);
+        if (dbg) dbg[3] = clock64();
+        if (dead) {
+            rg.ctl[4] = 1;
+            *reinterpret_cast<volatile int*>(&P.scal->abort) = 1;
+        } else {
+            // recycle the slots just read
+#pragma unroll
+            for (int i = 0; i < NV; ++i)
+#pragma unroll
+                for (int m = 0; m < kBarM; ++m) {
+                    const int j = lane + 32 * m;
+                    if (j < G) st_relaxed_u64(mine + i * kBarGrid + j, kIdle);
+                }
+        }
         __syncwarp();
         if (dbg) dbg[4] = clock64();
         if (FENCED) asm volatile("fence.acq_rel.gpu;" ::: "memory");
@@ -542,6 +650,7 @@ __device__ __forceinline__ void grid_allreduce(const Params& P, double* red, uns
             tot = warp_sum(tot);
             if (lane == 0) red[kRedTot + i] = tot;
         }
+        if (lane == 0) red[kRedTot + kBarVals] = rg.ctl[4] != 0 ? 1.0 : 0.0;
     }
     if (dbg) dbg[6] = clock64();
     consumer_sync<W>();
@@ -549,6 +658,7 @@ __device__ __forceinline__ void grid_allreduce(const Params& P, double* red, uns
 #pragma unroll
     for (int i = 0; i < NV; ++i) v[i] = red[kRedTot + i];
     ++count;
+    return red[kRedTot + kBarVals] != 0.0;
 }
 
 // Pure grid barrier (no payload), used after K3 to publish p: one relaxed atomic add on a
@@ -556,9 +666,10 @@ __device__ __forceinline__ void grid_allreduce(const Params& P, double* red, uns
 // also invalidates this SM's L1 so the K1 gathers see the new p).  About half the latency of
 // the push/poll exchange (1.5 k against 3.1 k cycles stand-alone): 148 atomics on one line
 // and 148 polling threads instead of 21 904 stores.  The counter (Scal::bar) is zeroed per
-// solve and only grows; `nbar` counts this CTA's arrivals.
+// solve and only grows; `nbar` counts this CTA's arrivals.  Returns true when the watchdog
+// tripped (same value in every consumer thread).
 template <int W>
-__device__ __forceinline__ void grid_barrier_counter(const Params& P, unsigned long long& nbar, int G,
+__device__ __forceinline__ bool grid_barrier_counter(const Params& P, const Ring& rg, unsigned long long& nbar, int G,
                                                      unsigned long long* dbg = nullptr) {
     if (dbg) dbg[0] = clock64();
     consumer_sync<W>();                    // all phase stores of the CTA happen-before the fence below
@@ -569,14 +680,16 @@ __device__ __forceinline__ void grid_barrier_counter(const Params& P, unsigned l
         asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(1ULL) : "memory");
         if (dbg) dbg[2] = clock64();
         const unsigned long long target = (++nbar) * (unsigned long long)G;
-        while (ld_relaxed_u64(ctr) < target) { }
+        bounded_spin(rg, [&] { return ld_relaxed_u64(ctr) >= target; });
         if (dbg) dbg[3] = clock64();
         if (dbg) dbg[4] = dbg[3];
         asm volatile("fence.acq_rel.gpu;" ::: "memory");
         if (dbg) { dbg[5] = clock64(); dbg[6] = dbg[5]; }
+        rg.red[kRedTot + kBarVals] = rg.ctl[4] != 0 ? 1.0 : 0.0;
     }
     consumer_sync<W>();
     if (dbg) dbg[7] = clock64();
+    return rg.red[kRedTot + kBarVals] != 0.0;
 }
 
 // ---------------------------------------------------------------- vector phases, vectors in global memory
@@ -592,19 +705,8 @@ __device__ __forceinline__ void st_cs_f64(double* p, double v) {
     asm volatile("st.global.cs.f64 [%0], %1;" :: "l"(p), "d"(v) : "memory");
 }
 
-// Optional L2 residency hints for the big-system path (option "l2_hints", off by default).  q
-// is written by K1 and read by K2 a whole matrix sweep (1.3 GB at config 4) later: its stores
-// ask the L2 to keep the lines (evict_last), the one read in K2 releases them (evict_first).
-// Measured at config 4: K2 55.6 k instead of 59.9 k cycles, but K3 28.2 k instead of 16.2 k
-// (r and p lose their place in the L2): a net loss, hence off.
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ void st_hint_f64(double* p, double v, uint64_t pol) {
-    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" :: "l"(p), "d"(v), "l"(pol) : "memory");
-}
+// q is read once in K2 a whole matrix sweep after K1 wrote it: when the matrix streams from HBM
+// that read carries an evict-first hint so the lines leave the L2 to p and r.
 __device__ __forceinline__ double ld_hint_f64(const double* p, uint64_t pol) {
     double v;
     asm volatile("ld.global.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol) : "memory");
@@ -718,7 +820,7 @@ __device__ __forceinline__ void phase_zero_x_tiles(const Params& P, long long tb
 
 // K1 with vectors in global memory: y = A x over this CTA's tiles, for the pass that starts at
 // ring position `pos`; returns this thread's partial of x.y when DOT.
-template <int W, int U, bool DOT>
+template <int W, int U, bool DOT, bool CMP, bool GF>
 __device__ __forceinline__ double phase_spmv_tiles(const Params& P, const Ring& rg, const double* x,
                                                    double* y, long long tb, int Tc, RingPos pos) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -727,10 +829,9 @@ __device__ __forceinline__ double phase_spmv_tiles(const Params& P, const Ring& 
         const long long row = (tb + j) * kTileRows + lane;
         double xr = 0.0;
         if (DOT && row < P.n) xr = ld_global_f64(x + row);      // early: off the critical path
-        const double acc = consume_tile<U>(rg, x, pos, j, lane);
+        const double acc = consume_tile<U, false, CMP, GF>(rg, x, pos, j, lane, (int)row);
         if (row < P.n) {
-            if (P.l2_stream & 2) st_hint_f64(y + row, acc, l2_policy_evict_last());
-            else y[row] = acc;
+            y[row] = acc;
             if (DOT) dot = fma(acc, xr, dot);
         }
     }

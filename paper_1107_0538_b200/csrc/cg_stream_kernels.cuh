@@ -29,24 +29,26 @@ __device__ __forceinline__ void decide_start(const Params& P, double rr, double 
     (void)warp
 
 // ---- cg_spmv: y = A x
-template <int W, int NP, int U>
+template <int W, int NP, int U, bool GF, bool CMP>
 __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_spmv(Params P, const double* x, double* y) {
     CGS_PROLOGUE(W);
-    ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, NP); return; }
-    phase_spmv_tiles<W, U, false>(P, rg, x, y, tb, Tc, RingPos{0u, 0u, 0u});
+    ring_init(P, rg);
+    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, 1, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
+    phase_spmv_tiles<W, U, false, CMP, GF>(P, rg, x, y, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
 // ---- stand-alone kernels of loop modes 1 (graph) and 2 (stepwise).  They read Params from
 // ---- device memory so that a captured graph survives across solves.
 
-template <int W, int NP, int U>
+template <int W, int NP, int U, bool GF, bool CMP>
 __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_init_spmv(const Params* __restrict__ dp) {
     const Params P = *dp;
     CGS_PROLOGUE(W);
-    ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, NP); return; }
-    phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, RingPos{0u, 0u, 0u});
+    ring_init(P, rg);
+    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, 1, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
+    phase_spmv_tiles<W, U, false, CMP, GF>(P, rg, P.x, P.q, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
 template <int W, int NP>
@@ -83,15 +85,16 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_init_scalars(con
     }
 }
 
-template <int W, int NP, int U>
+template <int W, int NP, int U, bool GF, bool CMP>
 __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks1_spmv_dot(const Params* __restrict__ dp, int s) {
     const Params P = *dp;
     if (P.scal->st[s].stop) return;
     CGS_PROLOGUE(W);
     if (cta == 0 && threadIdx.x == 0) P.scal->brk[s] = 0;
-    ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, 1, warp - W, NP); return; }
-    const double d = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, RingPos{0u, 0u, 0u});
+    ring_init(P, rg);
+    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, 1, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
+    const double d = phase_spmv_tiles<W, U, true, CMP, GF>(P, rg, P.p, P.q, tb, Tc, RingPos{0u, 0u, 0u});
     const double t = block_sum_w<W>(d, rg.red);
     if (threadIdx.x == 0) P.part0[cta] = t;
 }
@@ -157,13 +160,54 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks3_update_p(const 
 //        x, r, p, q (and D^-1) of those rows in registers from the prologue to the end; the
 //        only vector traffic left per iteration is the store of p and the gathers of K1.
 // R = 0: vectors in global memory (systems with more than R_max * 32 * W * G rows).
-// Scalars live in registers, identical in every CTA; three grid all-reduces per iteration
-// (after K1: p.q; after K2: r.r; after K3: a pure barrier that publishes p).
-template <int W, int NP, int U, int R, bool PRE>
+// Scalars live in registers, identical in every CTA.
+//
+// The synchronisations of one iteration, in order, are fixed HERE and nowhere else:
+//   plain loop   all-reduce (p.q) after K1, all-reduce (r.r) after K2, both carrying only their
+//                payload, then the counter barrier after K3 that publishes p;
+//   folded loop  (FOLD: R > 0, no preconditioner) all-reduce (p.q) after K1, then a FENCED
+//                all-reduce (r.r) after K2 that also publishes the {p, r} pairs the next K1
+//                gathers; K3 happens inside that K1.
+// grid_allreduce's slot recycling needs a fully fenced synchronisation strictly between any
+// all-reduce and the third all-reduce after it (see cg_stream.cuh); plan_is_safe checks that
+// for the cyclic sequence, and the call sites below take their kind from the plan.
+enum SyncKind { kArRelaxed = 0, kArFenced = 1, kCounter = 2 };
+template <bool FOLD> struct SyncPlan;
+template <> struct SyncPlan<false> { static constexpr int n = 3; static constexpr SyncKind seq[3] = {kArRelaxed, kArRelaxed, kCounter}; };
+template <> struct SyncPlan<true>  { static constexpr int n = 2; static constexpr SyncKind seq[2] = {kArRelaxed, kArFenced}; };
+
+template <class Plan> constexpr bool plan_is_safe() {
+    for (int i = 0; i < Plan::n; ++i) {
+        if (Plan::seq[i] == kCounter) continue;
+        int ars = 0; bool fenced = false;
+        for (int d = 1; d <= 4 * Plan::n && ars < 3; ++d) {       // walk on (cyclically) to the third all-reduce after i
+            const SyncKind k = Plan::seq[(i + d) % Plan::n];
+            if (k != kCounter) { ++ars; if (ars == 3) break; }
+            if (k == kArFenced || k == kCounter) fenced = true;
+        }
+        if (!fenced) return false;
+    }
+    return true;
+}
+static_assert(plan_is_safe<SyncPlan<false>>() && plan_is_safe<SyncPlan<true>>(), "all-reduce slots could be rewritten before their reset is ordered");
+
+// Step STEP of the plan: an all-reduce of v (NV values) or the payload-free counter barrier.
+template <int W, class Plan, int STEP, int NV>
+__device__ __forceinline__ bool iter_sync(const Params& P, const Ring& rg, unsigned& bcount, unsigned long long& nbar,
+                                          int cta, int G, double (&v)[NV], unsigned long long* dbg = nullptr) {
+    static_assert(STEP < Plan::n, "no such step");
+    if constexpr (Plan::seq[STEP] == kCounter) return grid_barrier_counter<W>(P, rg, nbar, G, dbg);
+    else return grid_allreduce<W, NV, Plan::seq[STEP] == kArFenced>(P, rg, bcount, cta, G, v, dbg);
+}
+
+template <int W, int NP, int U, bool GF, int R, bool PRE, bool FOLD, bool CMP>
 __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Params P) {
+    static_assert(!FOLD || (R > 0 && !PRE), "the folded loop needs the vectors in registers and no preconditioner");
+    using Plan = SyncPlan<FOLD>;
     CGS_PROLOGUE(W);
-    ring_init(rg);
-    if (warp >= W) { producer_loop(P, rg, tb, Tc, LLONG_MAX, warp - W, NP); return; }
+    ring_init(P, rg);
+    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, LLONG_MAX, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
     const int lane = threadIdx.x & 31;
     const bool lead = cta == 0 && threadIdx.x == 0;
     Scal* S = P.scal;
@@ -191,7 +235,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
 #pragma unroll
         for (int kk = 0; kk < R; ++kk) {
             const int j = warp + kk * W;
-            if (j < Tc) qv[kk] = consume_tile<U>(rg, P.x, pos, j, lane);
+            if (j < Tc) qv[kk] = consume_tile<U, false, CMP, GF>(rg, P.x, pos, j, lane, (int)((tb + j) * kTileRows + lane));
         }
 #pragma unroll
         for (int kk = 0; kk < R; ++kk) {
@@ -202,19 +246,22 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
             arr = fma(ri, ri, arr);
             if (PRE) { const double zi = dv[kk] * ri; pv[kk] = zi; arz = fma(ri, zi, arz); }
             else pv[kk] = ri;
-            P.p[row[kk]] = pv[kk];
+            if (FOLD) P.pr0[row[kk]] = make_double2(pv[kk], rv[kk]);      // the pair the first K1 gathers
+            else P.p[row[kk]] = pv[kk];
         }
     } else {
-        phase_spmv_tiles<W, U, false>(P, rg, P.x, P.q, tb, Tc, pos);
+        phase_spmv_tiles<W, U, false, CMP, GF>(P, rg, P.x, P.q, tb, Tc, pos);
+        asm volatile("" ::: "memory");                          // q below is what this thread just stored
         phase_init_tiles<W, PRE>(P, tb, Tc, arr, abb, arz);     // reads only this thread's own q
     }
     ++pass; pos = ring_next_pass(rg, pos, Tc);
     double rr, bb, rz;
+    bool dead;
     {
         double v[PRE ? 3 : 2];
         v[0] = arr; v[1] = abb;
         if (PRE) v[PRE ? 2 : 0] = arz;
-        grid_allreduce<W, (PRE ? 3 : 2), true>(P, rg.red, bcount, cta, G, v);
+        dead = grid_allreduce<W, (PRE ? 3 : 2), true>(P, rg, bcount, cta, G, v);
         rr = v[0]; bb = v[1]; rz = PRE ? v[PRE ? 2 : 0] : rr;
     }
     if (bb == 0.0) {
@@ -229,6 +276,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
     long long k = 0; int stop, status; double thresh;
     decide_start(P, rr, bb, &stop, &status, &thresh);
     if (PRE && S->diag_bad) { stop = 1; status = CG_BREAKDOWN; }
+    if (dead) { stop = 1; status = CG_ETIMEOUT; }
     if (lead && P.hist) P.hist[0] = sqrt(rr);
 
     // Optional trace (cg_set_trace): thread 0 of every CTA stamps clock64 at 8 points of each
@@ -238,10 +286,8 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
         ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
     unsigned long long full_wait = 0;
     if (tr) rg.acc = &full_wait;
-    // Folded loop (R > 0, no preconditioner, option "fold"): two grid synchronisations per
-    // iteration.  cur = which p buffer holds the p the next plain gather / fold would read.
-    const bool fold = R > 0 && !PRE && P.fold != 0;
-    bool have_beta = false;
+    // Folded loop: cur = which pair buffer holds the {p, r} the next K1 gathers; the first K1 runs
+    // with beta = 0, for which fma(beta, p, r) is r = p_0 to the bit.
     double beta_prev = 0.0;
     int cur = 0;
 #define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
@@ -251,23 +297,24 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
         double dot = 0.0;
         consumers_begin_pass(rg, pass);
         if constexpr (R > 0) {
-            const double* psrc = cur ? P.p2 : P.p;
-            if (fold && have_beta) {
+            if constexpr (FOLD) {
                 // K3 folded in: p = r + beta p for the rows this thread owns (registers, and
-                // the other p buffer for next iteration's gathers) ...
-                double* pdst = cur ? P.p : P.p2;
+                // the other pair buffer for next iteration's gathers) ...
+                const double2* psrc = cur ? P.pr1 : P.pr0;
+                double2* pdst = cur ? P.pr0 : P.pr1;
 #pragma unroll
                 for (int kk = 0; kk < R; ++kk) {
                     if (row[kk] < 0) continue;
                     pv[kk] = fma(beta_prev, pv[kk], rv[kk]);
-                    pdst[row[kk]] = pv[kk];
+                    pdst[row[kk]].x = pv[kk];
                 }
                 // ... and, recomputed on the fly, for every column the SpMV gathers
 #pragma unroll
                 for (int kk = 0; kk < R; ++kk) {
                     const int j = warp + kk * W;
                     if (j < Tc) {
-                        qv[kk] = consume_tile<U, true>(rg, psrc, pos, j, lane, P.r, beta_prev);
+                        qv[kk] = consume_tile<(U > 9 ? 9 : U), true, CMP, GF>(rg, reinterpret_cast<const double*>(psrc), pos, j, lane,
+                                                            (int)((tb + j) * kTileRows + lane), beta_prev);
                         if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
                     }
                 }
@@ -277,19 +324,20 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
                 for (int kk = 0; kk < R; ++kk) {
                     const int j = warp + kk * W;
                     if (j < Tc) {
-                        qv[kk] = consume_tile<U>(rg, psrc, pos, j, lane);
+                        qv[kk] = consume_tile<U, false, CMP, GF>(rg, P.p, pos, j, lane, (int)((tb + j) * kTileRows + lane));
                         if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
                     }
                 }
             }
         } else {
-            dot = phase_spmv_tiles<W, U, true>(P, rg, P.p, P.q, tb, Tc, pos);
+            dot = phase_spmv_tiles<W, U, true, CMP, GF>(P, rg, P.p, P.q, tb, Tc, pos);
         }
         ++pass; pos = ring_next_pass(rg, pos, Tc);
         CGS_STAMP(k, 1);
         double v1[1] = {dot};
-        grid_allreduce<W, 1, false>(P, rg.red, bcount, cta, G, v1);
+        dead = iter_sync<W, Plan, 0>(P, rg, bcount, nbar, cta, G, v1);
         CGS_STAMP(k, 2);
+        if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
         // scalar alpha (every CTA, same order, same value)
         const double pq = v1[0];
         if (!(pq > 0.0) || !finite_d(pq)) { stop = 1; status = CG_BREAKDOWN; break; }
@@ -298,6 +346,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
         arr = 0.0; arz = 0.0;
         if constexpr (R > 0) {
             const double na = -alpha;
+            double2* pnext = cur ? P.pr1 : P.pr0;              // FOLD: the buffer this K1 stored p into
 #pragma unroll
             for (int kk = 0; kk < R; ++kk) {
                 if (row[kk] < 0) continue;
@@ -305,7 +354,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
                 rv[kk] = fma(na, qv[kk], rv[kk]);
                 arr = fma(rv[kk], rv[kk], arr);
                 if (PRE) arz = fma(rv[kk], dv[kk] * rv[kk], arz);
-                if (fold) P.r[row[kk]] = rv[kk];          // gathered by the next K1
+                if (FOLD) pnext[row[kk]].y = rv[kk];          // gathered by the next K1
             }
         } else {
             phase_xr_tiles<W, PRE>(P, alpha, tb, Tc, arr, arz);
@@ -314,9 +363,9 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
         double v2[PRE ? 2 : 1];
         v2[0] = arr;
         if (PRE) v2[PRE ? 1 : 0] = arz;
-        if (fold) grid_allreduce<W, (PRE ? 2 : 1), true>(P, rg.red, bcount, cta, G, v2);      // publishes r and p
-        else      grid_allreduce<W, (PRE ? 2 : 1), false>(P, rg.red, bcount, cta, G, v2);
+        dead = iter_sync<W, Plan, 1>(P, rg, bcount, nbar, cta, G, v2);      // FOLD: fenced, publishes the pairs
         CGS_STAMP(k, 4);
+        if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
         // scalar beta, continue-condition
         const double rr_new = v2[0];
         const double rz_new = PRE ? v2[PRE ? 1 : 0] : rr_new;
@@ -328,28 +377,30 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
         if (lead && P.hist) P.hist[k] = res;
         if (res <= thresh) { stop = 1; status = CG_OK; break; }
         if (k >= P.maxit) { stop = 1; status = CG_MAXIT; break; }
-        if (fold) {                        // K3 happens inside the next K1
-            have_beta = true; beta_prev = beta;
+        if constexpr (FOLD) {              // K3 happens inside the next K1
+            beta_prev = beta;
             CGS_STAMP(k - 1, 6);
             CGS_STAMP(k - 1, 7);
-            continue;
-        }
-        // K3: p = r + beta p
-        if constexpr (R > 0) {
-#pragma unroll
-            for (int kk = 0; kk < R; ++kk) {
-                if (row[kk] < 0) continue;
-                const double zi = PRE ? rv[kk] * dv[kk] : rv[kk];
-                pv[kk] = fma(beta, pv[kk], zi);
-                P.p[row[kk]] = pv[kk];
-            }
         } else {
-            phase_p_tiles<W, PRE>(P, beta, tb, Tc);
+            // K3: p = r + beta p
+            if constexpr (R > 0) {
+#pragma unroll
+                for (int kk = 0; kk < R; ++kk) {
+                    if (row[kk] < 0) continue;
+                    const double zi = PRE ? rv[kk] * dv[kk] : rv[kk];
+                    pv[kk] = fma(beta, pv[kk], zi);
+                    P.p[row[kk]] = pv[kk];
+                }
+            } else {
+                phase_p_tiles<W, PRE>(P, beta, tb, Tc);
+            }
+            CGS_STAMP(k - 1, 6);
+            double none[1] = {0.0};
+            dead = iter_sync<W, Plan, Plan::n - 1>(P, rg, bcount, nbar, cta, G, none,      // publishes p
+                                                   (tr && k - 1 < P.trace_iters) ? tr + (k - 1) * kTraceSlots + 8 : nullptr);
+            CGS_STAMP(k - 1, 7);
+            if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
         }
-        CGS_STAMP(k - 1, 6);
-        grid_barrier_counter<W>(P, nbar, G,                               // publishes p
-                                (tr && k - 1 < P.trace_iters) ? tr + (k - 1) * kTraceSlots + 8 : nullptr);
-        CGS_STAMP(k - 1, 7);
     }
 #undef CGS_STAMP
     if constexpr (R > 0) {
