@@ -40,6 +40,33 @@ __global__ void k_stats(const int* __restrict__ rowptr, long long n, Scal* scal)
     }
 }
 
+// cg_create statistic: how many distinct 128-byte lines one warp-wide gather of the streamed
+// SpMV touches on average (lane l gathers x[col] of entry t of row 32 tile + l).  ~2.5 for a
+// stencil in natural ordering, ~30 for a random permutation: it decides how much of the SM's
+// L1 / shared-memory array the ring may take (geometry()).
+__global__ void k_gather_stats(const int* __restrict__ rp_pad, const int* __restrict__ colind, long long n,
+                               unsigned long long* lines, unsigned long long* requests) {
+    const int lane = threadIdx.x & 31;
+    const long long ntiles = (n + kTileRows - 1) / kTileRows;
+    const long long wstride = (long long)gridDim.x * (blockDim.x >> 5);
+    unsigned long long nl = 0, nr = 0;
+    for (long long t = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < ntiles; t += wstride) {
+        const long long row = t * kTileRows + lane;
+        const int rs = rp_pad[row], len = rp_pad[row + 1] - rs;
+        int maxlen = len;
+        for (int o = 16; o > 0; o >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, o));
+        for (int tt = 0; tt < maxlen; ++tt) {
+            const bool in = tt < len;
+            const int line = in ? (colind[rs + tt] >> 4) : -1 - lane;          // idle lanes: a private key each
+            const unsigned same = __match_any_sync(0xffffffffu, line);
+            const bool leader = in && (__ffs(same) - 1) == lane;
+            nl += __popc(__ballot_sync(0xffffffffu, leader));
+            nr += 1;
+        }
+    }
+    if (lane == 0) { atomicAdd(lines, nl); atomicAdd(requests, nr); }
+}
+
 __global__ void k_check_csr(const int* __restrict__ rowptr, const int* __restrict__ colind,
                             long long n, long long nnz, Scal* scal) {
     int bad = 0;
@@ -456,6 +483,8 @@ struct cg_handle {
     int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, pin_opt, compress_opt;
     int spin_budget_ms, inject_fault;
     int max_row_len, max_tile_nnz, tpr;
+    double lines_per_gather;               // cg_create statistic (k_gather_stats)
+    int smem_cap_kb;                       // option: 0 = auto
     bool dinv_ready;
     int grid_generic;                      // cooperative grid of the generic variant
     unsigned char* idx; size_t idx_bytes; bool idx_ready; int idx_codes;     // compressed index (borrowed buffer)
@@ -528,15 +557,28 @@ static Geo geometry(const cg_handle* h, bool cmp, int idx) {
         g.slot_bytes = (int)align_up((size_t)g.cap * 12u + (size_t)cgs::kRpInts * 4u, 128);
     }
     const size_t fixed = (size_t)cgs::kSmemTail + (cmp ? (size_t)cgs::kOffTabBytes : 0u);
+    g.from_hbm = (size_t)h->nnz * (cmp ? 9u : 12u) > h->l2_bytes / 2;
+    // How much of the SM's 256 KB L1 / shared-memory array a STREAMING ring may take.  What is
+    // left is the L1, and an L1 line is what an outstanding gather miss occupies: with 227 KB of
+    // ring the 28 KB of L1 allow ~220 lines in flight per SM, i.e. 7 warp-wide gathers when every
+    // lane hits its own line.  Measured (us per iteration, ring depth): config 3 (permuted) 32.9
+    // at 20 slots, 20.5 at 10-15; config 4 263 at 20 compressed slots (158 KB), 276 at 25, 295 at
+    // 10; config 2 streamed 11.8 at 20 plain slots, 12.6 at 15.
+    long long cap_bytes = h->smem_optin;
+    if (h->smem_cap_kb > 0) cap_bytes = (long long)h->smem_cap_kb * 1024;
+    else if (h->lines_per_gather > 8.0) cap_bytes = 132 * 1024;
+    else if (g.from_hbm) cap_bytes = 164 * 1024;
+    if (cap_bytes > h->smem_optin) cap_bytes = h->smem_optin;
     long long raw = ((long long)h->smem_optin - (long long)fixed) / g.slot_bytes;
+    const long long raw_stream = (cap_bytes - (long long)fixed) / g.slot_bytes;
     if (raw > cgs::kMaxSlots) raw = cgs::kMaxSlots;
     if (raw > h->max_slots) raw = h->max_slots;
     const long long tc_max = tiles_per_cta_max(h);
-    g.from_hbm = (size_t)h->nnz * (cmp ? 9u : 12u) > h->l2_bytes / 2;
     if (h->sms > cgs::kBarGrid || raw < 1) return g;
     if (h->pin_opt == 1 && !g.from_hbm && tc_max <= raw) {
         g.slots = (int)tc_max; g.pinned = (int)tc_max; g.stream_slots = 0; g.valid = true;
     } else if (NP > 0) {
+        if (raw > raw_stream && raw_stream >= 8) raw = raw_stream;      // never below the 8 slots that make a matrix streamable
         long long P = h->pin_opt >= 2 ? (h->pin_opt < tc_max ? h->pin_opt : tc_max) : 0;
         if (P > raw - 8) P = raw - 8 > 0 ? raw - 8 : 0;
         long long Q = raw - P;
@@ -692,6 +734,15 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     CKH(cudaStreamSynchronize(0));
     h->max_row_len = h->h_scal->max_row_len;
     h->max_tile_nnz = h->h_scal->max_tile_nnz;
+    if (nnz > 0) {
+        unsigned long long* cnt = reinterpret_cast<unsigned long long*>(h->part0);     // scratch until the first solve
+        CKH(cudaMemsetAsync(cnt, 0, 16, 0));
+        k_gather_stats<<<h->sms * 8, 256, 0, 0>>>(h->rp_pad, h->colind, h->n, cnt, cnt + 1);
+        CKH(cudaGetLastError());
+        unsigned long long hc[2] = {0, 0};
+        CKH(cudaMemcpy(hc, cnt, 16, cudaMemcpyDeviceToHost));
+        h->lines_per_gather = hc[1] ? (double)hc[0] / (double)hc[1] : 0.0;
+    }
     const double mean = (double)nnz / (double)n;
     h->tpr = mean <= 3 ? 2 : mean <= 6 ? 4 : mean <= 40 ? 8 : mean <= 96 ? 16 : 32;
     int rc = setup_generic(h);
@@ -807,6 +858,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         h->pin_opt = (int)value; drop_graph();
         return CG_OK;
     }
+    if (!strcmp(name, "smem_cap_kb")) { if (value < 0 || value > 227) return CG_EINVAL; h->smem_cap_kb = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
@@ -851,6 +903,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
     else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
     else if (!strcmp(name, "from_hbm")) *value = g.from_hbm ? 1 : 0;
+    else if (!strcmp(name, "lines_per_gather_x100")) *value = (int64_t)(h->lines_per_gather * 100.0 + 0.5);
     else return CG_EINVAL;
     return CG_OK;
 }

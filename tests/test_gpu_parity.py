@@ -236,7 +236,7 @@ def test_solve_long_rows_streamed(cgmod, orc, half_band):
             cg.set_option("loop", loop)
             x, res = cg.solve(dev(b), rtol=1e-10, maxit=n)
             check_solve_parity(res, x, ref)
-            outs.append((variant, x.cpu().numpy().copy()))
+            outs.append((cg.info("spmv"), x.cpu().numpy().copy()))
     for (va_, xa), (vb_, xb) in zip(outs[::2], outs[1::2]):
         assert va_ == vb_ and np.array_equal(xa, xb)             # persistent == graph twin, per variant
     cg.set_option("compress", 1)
