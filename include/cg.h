@@ -172,9 +172,20 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               iteration, copy it there once per solve and keep it; 0 = stream everything
  *               every iteration; k >= 2 = pin k tiles per CTA and stream the rest (a mixed
  *               split, kept for tests and measurements)
+ *   "algo"      0 (default) = the textbook recurrence of cg_solve above, three grid
+ *               synchronisations per iteration.  1 = Chronopoulos-Gear single-reduction CG
+ *               (SURVEY.md 8(f) rank 2): w = A r, ONE all-reduce of (r.r, w.r) and one barrier
+ *               that publishes r per iteration; same iterates in exact arithmetic, different
+ *               rounding (held to the same parity bands in the tests, never the default).
+ *               Applies to loop 0 with the vectors in registers and no preconditioner;
+ *               otherwise the textbook path runs (cg_get_info "algo" tells which).
  *   "compress"  1 (default) = use the compressed index once cg_compress_index has built it;
  *               0 = plain CSR slots
  *   "ring_slots" cap on the ring depth (8..64)
+ *   "smem_cap_kb" cap (KB) on the shared memory a STREAMING ring may take; what is left of the
+ *               SM's 256 KB array is L1, whose lines hold the outstanding gather misses.
+ *               0 (default) = auto: 132 KB when gathers are irregular (> 8 lines per warp-wide
+ *               gather), 164 KB when the matrix streams from HBM, else all of it
  *   "lookahead" tiles the producers may prefetch of an iteration the consumers have not
  *               started (default unlimited: the ring is refilled across the grid barriers)
  *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant
@@ -186,7 +197,8 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
  * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "pinned_tiles", "slot_bytes",
- * "resident_rows", "fold", "compressed", "index_codes", "from_hbm".
+ * "resident_rows", "fold", "algo", "compressed", "index_codes", "from_hbm", "lines_per_gather_x100"
+ * (cg_create statistic: 128-byte lines one warp-wide gather touches on average, times 100).
  * Unknown names return CG_EINVAL. */
 int cg_set_option(cg_handle* h, const char* name, int64_t value);
 int cg_get_info(cg_handle* h, const char* name, int64_t* value);

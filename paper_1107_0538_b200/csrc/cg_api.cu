@@ -424,6 +424,7 @@ struct StreamFns {
     const void* init_spmv[2]; const void* init_residual; const void* init_scalars;
     const void* k1[2]; const void* k2; const void* k3;
     const void* persistent[2][kNumPersistent];
+    const void* cg1[2][2];                 // option "algo" = 1 (Chronopoulos-Gear): [cmp][R == 4]
 };
 
 template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(StreamFns& f) {
@@ -439,6 +440,8 @@ template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(Stre
     f.persistent[c][kR4]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, false, CMP>;
     f.persistent[c][kR4Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, true, false, CMP>;
     f.persistent[c][kR4Fold]   = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, true, CMP>;
+    f.cg1[c][0] = (const void*)cgs::ks_persistent_cg1<W, NP, U, GF, 2, CMP>;
+    f.cg1[c][1] = (const void*)cgs::ks_persistent_cg1<W, NP, U, GF, 4, CMP>;
 }
 template <int W, int NP, int U, bool GF> static StreamFns make_stream_fns() {
     StreamFns f;
@@ -481,7 +484,7 @@ struct cg_handle {
     int sms, smem_optin, clock_khz;
     size_t l2_bytes;
     int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, pin_opt, compress_opt;
-    int spin_budget_ms, inject_fault;
+    int spin_budget_ms, inject_fault, algo_opt;
     int max_row_len, max_tile_nnz, tpr;
     double lines_per_gather;               // cg_create statistic (k_gather_stats)
     int smem_cap_kb;                       // option: 0 = auto
@@ -642,6 +645,12 @@ static bool fold_effective(const cg_handle* h, int v, int precond, const Geo& g)
     return gathers <= 500.0;
 }
 
+// Option "algo" = 1 (Chronopoulos-Gear) applies to the persistent streamed kernel with the vectors
+// in registers and no preconditioner; everything else runs the textbook recurrence.
+static bool algo1_effective(const cg_handle* h, int v, int precond) {
+    return h->algo_opt == 1 && h->loop == 0 && !precond && resident_rows(h, v) > 0;
+}
+
 static void fill_params(const cg_handle* h, Params* P, const double* b, double* x, double rtol,
                         long long maxit, double* hist, int precond, int variant, const Geo& g) {
     memset(P, 0, sizeof(*P));
@@ -757,6 +766,8 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
             for (const void* fn : two) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
             for (int k = 0; k < kNumPersistent; ++k)
                 CKH(cudaFuncSetAttribute(f.persistent[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
+            for (int k = 0; k < 2; ++k)
+                CKH(cudaFuncSetAttribute(f.cg1[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
         }
     }
     *out = h;
@@ -858,6 +869,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         h->pin_opt = (int)value; drop_graph();
         return CG_OK;
     }
+    if (!strcmp(name, "algo")) { if (value < 0 || value > 1) return CG_EINVAL; h->algo_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "smem_cap_kb")) { if (value < 0 || value > 227) return CG_EINVAL; h->smem_cap_kb = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
@@ -900,6 +912,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "slot_bytes")) *value = v >= 2 ? g.slot_bytes : 0;
     else if (!strcmp(name, "resident_rows")) *value = resident_rows(h, v);
     else if (!strcmp(name, "fold")) *value = fold_effective(h, v, 0, g) ? 1 : 0;
+    else if (!strcmp(name, "algo")) *value = algo1_effective(h, v, 0) ? 1 : 0;
     else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
     else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
     else if (!strcmp(name, "from_hbm")) *value = g.from_hbm ? 1 : 0;
@@ -1063,9 +1076,9 @@ static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol,
                            : R == 2 ? (precond ? kR2Jacobi : fold ? kR2Fold : kR2)
                                     : (precond ? kR4Jacobi : fold ? kR4Fold : kR4);
             h->last_resident = R; h->last_fold = fold ? 1 : 0;
+            const void* fn = algo1_effective(h, v, precond) ? f.cg1[g.cmp][R == 4 ? 1 : 0] : f.persistent[g.cmp][kind];
             CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));        // arm the all-reduce slots
-            CK(cudaLaunchCooperativeKernel(f.persistent[g.cmp][kind], dim3(G), dim3(32 * (f.W + f.NP)),
-                                           args, g.smem, st));
+            CK(cudaLaunchCooperativeKernel(fn, dim3(G), dim3(32 * (f.W + f.NP)), args, g.smem, st));
         }
         h->launches += 1;
     } else {

@@ -413,4 +413,160 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
     if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(rr); }
 }
 
+// ---- option "algo" = 1: Chronopoulos-Gear conjugate gradients (second half).
+// The same Krylov iteration with ONE reduction per step: w = A r is formed instead of q = A p, the
+// two inner products gamma = r.r and delta = w.r share one all-reduce, and s = A p follows from the
+// recurrence s = w + beta s.  Per iteration (G. Meurant's form of Chronopoulos & Gear 1989):
+//     p = r + beta p ; s = w + beta s ; x += alpha p ; r -= alpha s          (registers of the owner)
+//     -- counter barrier: r is published --
+//     w = A r  fused with the partials of gamma' = r.r and delta = w.r        (K1)
+//     -- all-reduce (gamma', delta) --
+//     beta = gamma' / gamma ; alpha = gamma' / (delta - beta gamma' / alpha)   (the denominator is p'.A p')
+// Two grid synchronisations per iteration instead of three, 8-byte gathers as in the textbook
+// loop.  In exact arithmetic the iterates are those of the textbook recurrence;
+// in floating point they differ by rounding, so this is an OPTION, never the default: it is held
+// to the same parity bands against the same oracle (tests) and reported beside the textbook path.
+// k counts in-loop SpMVs as everywhere (the prologue has two: A x0 and A r0); hist[k] = ||r_k||.
+// Vectors in registers only (R > 0), no preconditioner; the host falls back to the textbook
+// kernel otherwise.
+struct SyncPlanCG1 { static constexpr int n = 2; static constexpr SyncKind seq[2] = {kCounter, kArRelaxed}; };
+static_assert(plan_is_safe<SyncPlanCG1>(), "all-reduce slots could be rewritten before their reset is ordered");
+
+template <int W, int NP, int U, bool GF, int R, bool CMP>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(Params P) {
+    static_assert(R > 0, "vectors in registers");
+    using Plan = SyncPlanCG1;
+    CGS_PROLOGUE(W);
+    ring_init(P, rg);
+    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, LLONG_MAX, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
+    const int lane = threadIdx.x & 31;
+    const bool lead = cta == 0 && threadIdx.x == 0;
+    Scal* S = P.scal;
+    unsigned bcount = 0;
+    unsigned long long nbar = 0;
+    unsigned long long pass = 0;
+    RingPos pos{0u, 0u, 0u};
+    double xr[R], rv[R], pv[R], sv[R], wv[R];
+    long long row[R];
+    double* const rpub = P.p;                 // the published copy of r that K1 gathers
+
+    // prologue: r0 = b - A x0 (published), then w0 = A r0 with gamma0 = r0.r0, delta0 = w0.r0, b.b
+    double abb = 0.0;
+    consumers_begin_pass(rg, pass);
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        const long long i = (tb + j) * kTileRows + lane;
+        row[kk] = (j < Tc && i < P.n) ? i : -1;
+        xr[kk] = 0.0; rv[kk] = 0.0; pv[kk] = 0.0; sv[kk] = 0.0; wv[kk] = 0.0;
+        double bi = 0.0;
+        if (row[kk] >= 0) { xr[kk] = P.x[i]; bi = P.b[i]; }
+        rv[kk] = bi;                           // b for now
+    }
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        double q = 0.0;
+        if (j < Tc) q = consume_tile<U, false, CMP, GF>(rg, P.x, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+        if (row[kk] >= 0) {
+            abb = fma(rv[kk], rv[kk], abb);
+            rv[kk] = rv[kk] - q;
+            rpub[row[kk]] = rv[kk];
+        }
+    }
+    ++pass; pos = ring_next_pass(rg, pos, Tc);
+    double none[1] = {0.0};
+    bool dead = iter_sync<W, Plan, 0>(P, rg, bcount, nbar, cta, G, none);          // r0 is published
+    double agam = 0.0, adel = 0.0;
+    consumers_begin_pass(rg, pass);
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        if (j < Tc) wv[kk] = consume_tile<U, false, CMP, GF>(rg, rpub, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+        if (row[kk] >= 0) { agam = fma(rv[kk], rv[kk], agam); adel = fma(wv[kk], rv[kk], adel); }
+    }
+    ++pass; pos = ring_next_pass(rg, pos, Tc);
+    double gam, del, bb;
+    {
+        double v[3] = {agam, adel, abb};
+        dead = grid_allreduce<W, 3, true>(P, rg, bcount, cta, G, v) || dead;
+        gam = v[0]; del = v[1]; bb = v[2];
+    }
+    if (bb == 0.0) {
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) xr[kk] = 0.0;
+        gam = 0.0;
+    }
+    long long k = 0; int stop, status; double thresh;
+    decide_start(P, gam, bb, &stop, &status, &thresh);
+    if (dead) { stop = 1; status = CG_ETIMEOUT; }
+    if (lead && P.hist) P.hist[0] = sqrt(gam);
+    double alpha = 0.0, beta = 0.0;
+    if (!stop) {
+        if (!(del > 0.0) || !finite_d(del)) { stop = 1; status = CG_BREAKDOWN; }      // p0.A p0 = r0.A r0
+        else alpha = gam / del;
+    }
+    unsigned long long* tr = (P.trace && threadIdx.x == 0)
+        ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
+#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
+    while (!stop) {
+        // trace slots keep the textbook kernel's meaning as far as it goes: 0 start, 1 K1 done, 2 past the
+        // all-reduce, 3..5 scalars, 6 vector updates done, 7 past the publish barrier of the NEXT K1's operand
+        // vector updates (the textbook's K3 and K2 in one pass over the registers)
+        const double na = -alpha;
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            if (row[kk] < 0) continue;
+            pv[kk] = fma(beta, pv[kk], rv[kk]);
+            sv[kk] = fma(beta, sv[kk], wv[kk]);
+            xr[kk] = fma(alpha, pv[kk], xr[kk]);
+            rv[kk] = fma(na, sv[kk], rv[kk]);
+            rpub[row[kk]] = rv[kk];
+        }
+        CGS_STAMP(k, 6);
+        dead = iter_sync<W, Plan, 0>(P, rg, bcount, nbar, cta, G, none,               // publishes r
+                                     (tr && k < P.trace_iters) ? tr + k * kTraceSlots + 8 : nullptr);
+        CGS_STAMP(k, 7);
+        if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
+        // K1: w = A r, partials of gamma' = r.r and delta = w.r
+        CGS_STAMP(k, 0);
+        agam = 0.0; adel = 0.0;
+        consumers_begin_pass(rg, pass);
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            const int j = warp + kk * W;
+            if (j < Tc) {
+                wv[kk] = consume_tile<U, false, CMP, GF>(rg, rpub, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+                if (row[kk] >= 0) { agam = fma(rv[kk], rv[kk], agam); adel = fma(wv[kk], rv[kk], adel); }
+            }
+        }
+        ++pass; pos = ring_next_pass(rg, pos, Tc);
+        CGS_STAMP(k, 1);
+        double v2[2] = {agam, adel};
+        dead = iter_sync<W, Plan, 1>(P, rg, bcount, nbar, cta, G, v2);
+        CGS_STAMP(k, 2);
+        if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
+        const double gam_new = v2[0];
+        del = v2[1];
+        const double res = sqrt(gam_new);
+        k += 1;
+        if (lead && P.hist) P.hist[k] = res;
+        if (res <= thresh) { gam = gam_new; stop = 1; status = CG_OK; break; }
+        if (k >= P.maxit) { gam = gam_new; stop = 1; status = CG_MAXIT; break; }
+        beta = gam_new / gam;
+        const double denom = del - beta * gam_new / alpha;       // = p'.A p' for the next direction
+        gam = gam_new;
+        if (!(denom > 0.0) || !finite_d(denom)) { stop = 1; status = CG_BREAKDOWN; break; }
+        alpha = gam / denom;
+        CGS_STAMP(k - 1, 5);
+    }
+#undef CGS_STAMP
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk)
+        if (row[kk] >= 0) P.x[row[kk]] = xr[kk];
+    if (threadIdx.x == 0) consumers_stop(rg, pass);
+    if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(gam); }
+}
+
 }  // namespace cgs

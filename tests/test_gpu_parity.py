@@ -562,6 +562,48 @@ def test_generic_ctas_per_sm(bound, orc, ctas):
         B.cg.set_option(k, v)
 
 
+# ---------------------------------------------------------------- single-reduction CG (8(f) rank 2, second half)
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_single_reduction_cg_parity(bound, orc, cfg):
+    """Option "algo" = 1: Chronopoulos-Gear CG (one all-reduce + one publish barrier per iteration).
+    Same Krylov iteration, different rounding: it must pass the same four bands against the same
+    (unchanged) oracle as the textbook path, and return an x whose true residual, computed with the
+    oracle's SpMV, meets rtol."""
+    B = bound(cfg)
+    p = B.p
+    B.cg.set_option("loop", 0)
+    B.cg.set_option("algo", 1)
+    assert B.cg.info("algo") == 1
+    ref = oracle_solve(orc, p, ("cg", cfg))
+    x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+    check_solve_parity(res, x, ref)
+    true_r = p.b - orc.spmv_ld(p.rowptr, p.colind, p.vals, x.cpu().numpy())
+    assert np.linalg.norm(true_r) / np.linalg.norm(p.b) <= 2 * p.rtol
+    x2, res2 = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+    assert torch.equal(x, x2) and torch.equal(res.hist, res2.hist)        # reproducible
+    # conventions hold here too
+    x3, r3 = B.cg.solve(B.b, rtol=0.0, maxit=5)
+    r5 = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=0.0, maxit=5)
+    assert r3.iters == 5 and r3.status == 1
+    assert np.linalg.norm(x3.cpu().numpy() - r5.x) / np.linalg.norm(r5.x) < 1e-12
+    x4, r4 = B.cg.solve(torch.zeros_like(B.b), x0=torch.ones_like(B.b), rtol=1e-10, maxit=10)
+    assert r4.iters == 0 and r4.status == 0 and float(x4.abs().max()) == 0.0
+    B.cg.set_option("loop", 1)
+    assert B.cg.info("algo") == 0                                          # graph twin: textbook only
+    B.cg.set_option("loop", 0)
+    B.cg.set_option("algo", 0)
+
+
+def test_single_reduction_cg_breakdown(bound, cgmod):
+    B = bound(0)
+    neg = cgmod.CG(dev(B.p.rowptr), dev(B.p.colind), dev(-B.p.vals))
+    neg.set_option("algo", 1)
+    x, res = neg.solve(B.b, rtol=1e-10, maxit=10)
+    assert res.status == 2 and res.iters == 0
+    neg.close()
+
+
 # ---------------------------------------------------------------- watchdog
 
 @pytest.mark.parametrize("compress,loop,spmv", [(1, 0, 0), (0, 0, 0), (0, 2, 3), (1, 1, 2)])
