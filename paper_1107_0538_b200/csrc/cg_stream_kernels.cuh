@@ -425,7 +425,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
 // Two grid synchronisations per iteration instead of three, 8-byte gathers as in the textbook
 // loop.  In exact arithmetic the iterates are those of the textbook recurrence;
 // in floating point they differ by rounding, so this is an OPTION, never the default: it is held
-// to the same parity bands against the same oracle (tests) and reported beside the textbook path.
+// to the same parity bands as the textbook path in the tests and reported beside it.
 // k counts in-loop SpMVs as everywhere (the prologue has two: A x0 and A r0); hist[k] = ||r_k||.
 // Vectors in registers only (R > 0), no preconditioner; the host falls back to the textbook
 // kernel otherwise.
