@@ -103,32 +103,40 @@ constexpr size_t kIdxHashOff = 1024;                 // kIdxHash long longs of s
 constexpr size_t kIdxRecOff = 1024 + 8 * kIdxHash;   // records (a multiple of 128)
 
 // Pass 1: the set of distinct offsets d = col - row, at most kMaxCodes of them (else overflow).
+// Offset 0 is always a member (the records pad short rows with its code: a padding gather then
+// reads x[row], a valid address).
+__device__ __forceinline__ bool idx_insert(long long* table, Scal* scal, long long d) {
+    unsigned slot = (unsigned)((unsigned long long)d * 0x9E3779B97F4A7C15ULL >> 54);      // top 10 bits
+    for (int probes = 0; probes < kIdxHash; ++probes, slot = (slot + 1) & (kIdxHash - 1)) {
+        long long cur = table[slot];                     // a stale "empty" is settled by the CAS
+        if (cur == d) return true;
+        if (cur == kIdxEmpty) {
+            cur = (long long)atomicCAS(reinterpret_cast<unsigned long long*>(table + slot),
+                                       (unsigned long long)kIdxEmpty, (unsigned long long)d);
+            if (cur == kIdxEmpty) {
+                if (atomicAdd(&scal->idx_count, 1) + 1 > cgs::kMaxCodes) scal->idx_overflow = 1;
+                return true;
+            }
+            if (cur == d) return true;
+        }
+    }
+    scal->idx_overflow = 1;
+    return false;
+}
+
 __global__ void k_idx_collect(const int* __restrict__ rowptr, const int* __restrict__ colind, long long n,
                               long long* table, Scal* scal) {
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t0 == 0) idx_insert(table, scal, 0);
+    for (long long i = t0; i < n; i += stride) {
         if (*reinterpret_cast<volatile int*>(&scal->idx_overflow)) return;
         long long last = kIdxEmpty;
         for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
             const long long d = (long long)colind[k] - i;
             if (d == last) continue;
             last = d;
-            unsigned slot = (unsigned)((unsigned long long)d * 0x9E3779B97F4A7C15ULL >> 54);      // top 10 bits
-            int probes = 0;
-            for (;; slot = (slot + 1) & (kIdxHash - 1)) {
-                long long cur = table[slot];                     // a stale "empty" is settled by the CAS
-                if (cur == d) break;
-                if (cur == kIdxEmpty) {
-                    cur = (long long)atomicCAS(reinterpret_cast<unsigned long long*>(table + slot),
-                                               (unsigned long long)kIdxEmpty, (unsigned long long)d);
-                    if (cur == kIdxEmpty) {
-                        if (atomicAdd(&scal->idx_count, 1) + 1 > cgs::kMaxCodes) scal->idx_overflow = 1;
-                        break;
-                    }
-                    if (cur == d) break;
-                }
-                if (++probes >= kIdxHash) { scal->idx_overflow = 1; return; }
-            }
+            if (!idx_insert(table, scal, d)) return;
         }
     }
 }
@@ -148,7 +156,8 @@ __global__ void k_idx_sort(const long long* __restrict__ table, int* __restrict_
 
 // Pass 3 (one warp per tile): the tile's record = 33 u16 row starts relative to the tile,
 // [33] = parity of the tile's first entry (the vals span starts at an even entry), then the
-// codes transposed: entry t of the tile's row l at byte 80 + 32 t + l.
+// codes transposed and packed: the codes of entries 4 g .. 4 g + 3 of the tile's row l are the
+// bytes (low to high) of the 32-bit word at byte 80 + 4 (32 g + l).
 __global__ void k_idx_build(const int* __restrict__ rp_pad, const int* __restrict__ colind, long long n,
                             const int* __restrict__ off, int ncodes, unsigned char* __restrict__ rec, int rec_stride) {
     __shared__ int so[cgs::kMaxCodes];
@@ -157,7 +166,9 @@ __global__ void k_idx_build(const int* __restrict__ rp_pad, const int* __restric
     const int lane = threadIdx.x & 31;
     const long long ntiles = (n + kTileRows - 1) / kTileRows;
     const long long wstride = (long long)gridDim.x * (blockDim.x >> 5);
-    const int maxlen = (rec_stride - cgs::kRecHdr) / 32;
+    const int nwords = (rec_stride - cgs::kRecHdr) / 128;
+    int pad = 0;                                       // the code of offset 0 (always in the table)
+    { int lo = 0, hi = ncodes - 1; while (lo < hi) { const int mid = (lo + hi) >> 1; if (so[mid] < 0) lo = mid + 1; else hi = mid; } pad = lo; }
     for (long long t = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); t < ntiles; t += wstride) {
         const long long row = t * kTileRows + lane;
         const int s = rp_pad[t * kTileRows];
@@ -167,15 +178,21 @@ __global__ void k_idx_build(const int* __restrict__ rp_pad, const int* __restric
         hd[lane] = (unsigned short)(rs - s);
         if (lane < 8) hd[32 + lane] = lane == 0 ? (unsigned short)(rp_pad[t * kTileRows + kTileRows] - s)
                                     : lane == 1 ? (unsigned short)(s & 1) : (unsigned short)0;
-        for (int tt = 0; tt < maxlen; ++tt) {
-            int code = 0;
-            if (tt < re - rs) {
-                const int d = (int)((long long)colind[rs + tt] - row);
-                int lo = 0, hi = ncodes - 1;
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (so[mid] < d) lo = mid + 1; else hi = mid; }
-                code = lo;
+        unsigned* words = reinterpret_cast<unsigned*>(r + cgs::kRecHdr);
+        for (int g = 0; g < nwords; ++g) {
+            unsigned w = 0;
+            for (int b = 0; b < 4; ++b) {
+                const int tt = 4 * g + b;
+                int code = pad;
+                if (tt < re - rs) {
+                    const int d = (int)((long long)colind[rs + tt] - row);
+                    int lo = 0, hi = ncodes - 1;
+                    while (lo < hi) { const int mid = (lo + hi) >> 1; if (so[mid] < d) lo = mid + 1; else hi = mid; }
+                    code = lo;
+                }
+                w |= (unsigned)code << (8 * b);
             }
-            r[cgs::kRecHdr + tt * 32 + lane] = (unsigned char)code;
+            words[g * 32 + lane] = w;
         }
     }
 }
@@ -533,7 +550,9 @@ static int setup_generic(cg_handle* h) {
 static long long tiles_per_cta_max(const cg_handle* h) {
     return ((h->n + kTileRows - 1) / kTileRows + h->sms - 1) / h->sms;
 }
-static int rec_stride_of(const cg_handle* h) { return (int)align_up((size_t)cgs::kRecHdr + 32u * (size_t)h->max_row_len, 16); }
+static int rec_stride_of(const cg_handle* h) { return cgs::kRecHdr + 128 * ((h->max_row_len + 3) / 4); }
+// the shared-memory copy of the offset table: 128 bytes when the matrix names <= 32 offsets, else 1 KB
+static int offtab_entries(const cg_handle* h) { return h->idx_codes <= cgs::kOffTabSmall ? cgs::kOffTabSmall : cgs::kMaxCodes; }
 static bool use_cmp(const cg_handle* h) { return h->idx_ready && h->compress_opt != 0; }
 
 // Ring geometry of streamed variant `idx` from the matrix statistics.  A slot holds the largest
@@ -559,7 +578,7 @@ static Geo geometry(const cg_handle* h, bool cmp, int idx) {
         if (g.cap < 4) g.cap = 4;
         g.slot_bytes = (int)align_up((size_t)g.cap * 12u + (size_t)cgs::kRpInts * 4u, 128);
     }
-    const size_t fixed = (size_t)cgs::kSmemTail + (cmp ? (size_t)cgs::kOffTabBytes : 0u);
+    const size_t fixed = (size_t)cgs::kSmemTail + (cmp ? (size_t)offtab_entries(h) * 4u : 0u);
     g.from_hbm = (size_t)h->nnz * (cmp ? 9u : 12u) > h->l2_bytes / 2;
     // How much of the SM's 256 KB L1 / shared-memory array a STREAMING ring may take.  What is
     // left is the L1, and an L1 line is what an outstanding gather miss occupies: with 227 KB of
@@ -670,7 +689,7 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     P->pr0 = reinterpret_cast<double2*>(h->r);
     P->pr1 = reinterpret_cast<double2*>(h->q);
     P->l2_stream = g.from_hbm ? 1 : 0;
-    P->cmp = g.cmp; P->rec_stride = g.rec_stride;
+    P->cmp = g.cmp; P->rec_stride = g.rec_stride; P->ncodes_smem = offtab_entries(h);
     P->idx_off = h->idx ? reinterpret_cast<const int*>(h->idx + kIdxTableOff) : nullptr;
     P->idx_rec = h->idx ? h->idx + kIdxRecOff : nullptr;
     P->spin_budget = (long long)h->spin_budget_ms * (long long)h->clock_khz;

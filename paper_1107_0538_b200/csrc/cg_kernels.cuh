@@ -95,7 +95,8 @@ struct Params {
     int l2_stream;        // 1: the matrix does not fit the L2 -> evict-first hint on its copies
     // compressed index (cg_compress_index): one record per tile, see cg_stream.cuh
     int cmp;              // 1: slots hold {vals span, index record}
-    int rec_stride;       // bytes per record: 80 + 32 * (longest row), a multiple of 16
+    int rec_stride;       // bytes per record: 80 + 128 * ceil(longest row / 4)
+    int ncodes_smem;      // entries of the offset table copied into shared memory (32 or 256)
     const unsigned char* idx_rec;   // records, tile t at idx_rec + t * rec_stride
     const int* idx_off;   // kMaxCodes column offsets (col - row) named by the codes
     long long spin_budget;          // cycles any device-side spin may last before the watchdog trips

@@ -56,6 +56,7 @@ constexpr int kRedTot = 96;          // red[0..95]: per-warp partials (3 values 
 constexpr int kRecHdr = 80;          // compressed index record: 33 u16 row starts, [33] = s & 1, padded to 80 bytes
 constexpr int kMaxCodes = 256;       // distinct column offsets a compressed index can name
 constexpr int kOffTabBytes = kMaxCodes * 4;
+constexpr int kOffTabSmall = 32;     // with <= 32 codes (the stencils) the shared-memory copy of the table takes 128 bytes
 
 // W consumer warps + NP producer warps per CTA; W + NP is a multiple of 4 so the warps spread
 // evenly over the SM's four sub-partitions (their register files bound the registers per thread).
@@ -77,6 +78,8 @@ struct Ring {
     const int* offtab;                // compressed index: column offset per code (shared-memory copy)
     int S, slot_bytes, cap;
     int P, Q;                         // pinned slots [0, P) and streaming slots [P, P + Q), P + Q <= S
+    int rec_words;                    // compressed index: 32-bit code words per lane in a record
+    int n;                            // rows of the matrix
     long long budget;                 // cycles a spin may last
     Scal* scal;
     unsigned long long* acc;          // optional: cycles this thread waited on full barriers (trace)
@@ -97,7 +100,7 @@ struct Ring {
 __device__ __forceinline__ Ring ring_view(const Params& P, unsigned char* dyn) {
     Ring rg;
     rg.S = P.slots; rg.slot_bytes = P.slot_bytes; rg.cap = P.cap; rg.acc = nullptr;
-    rg.P = P.pinned; rg.Q = P.stream_slots;
+    rg.P = P.pinned; rg.Q = P.stream_slots; rg.rec_words = (P.rec_stride - kRecHdr) / 128; rg.n = (int)P.n;
     rg.budget = P.spin_budget; rg.scal = P.scal;
     rg.slots = dyn;
     unsigned char* tail = dyn + (size_t)P.slots * P.slot_bytes;
@@ -118,7 +121,7 @@ __device__ __forceinline__ void ring_init(const Params& P, const Ring& rg) {
         rg.tag[threadIdx.x] = 0u;
     }
     if (threadIdx.x < 8) rg.ctl[threadIdx.x] = 0;
-    if (P.cmp && threadIdx.x < kMaxCodes) const_cast<int*>(rg.offtab)[threadIdx.x] = P.idx_off[threadIdx.x];
+    if (P.cmp && (int)threadIdx.x < P.ncodes_smem) const_cast<int*>(rg.offtab)[threadIdx.x] = P.idx_off[threadIdx.x];
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -369,8 +372,9 @@ __device__ __forceinline__ double2 ld_global_f64x2(const double2* p) {
 // flight.  Padding entries (k >= ke) use value 0 and column 0.
 //
 // CMP: the slot holds the compressed index record: row bounds are u16 relative to the tile,
-// entry t of lane l has its code at byte [t * 32 + l] (transposed at setup: conflict-free
-// loads) and its column is row + offtab[code].
+// the codes of lane l's entries 4 g .. 4 g + 3 are the bytes of the 32-bit word [g * 32 + l]
+// (transposed and packed at setup: one conflict-free load fetches four codes) and an entry's
+// column is row + offtab[code].
 //
 // FOLD: the gathered operand is not stored anywhere yet: it is p_new[c] = fma(beta, p_old[c],
 // r[c]), the very expression K3 evaluates for row c, recomputed here by every thread that
@@ -402,12 +406,14 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
     int ks, ke;
     const double* sv = rg.vals(slot);
     const int* sc = nullptr;
-    const unsigned char* sb = nullptr;
+    const unsigned* sw = nullptr;
+    int gmax = 0;
     if constexpr (CMP) {
         const unsigned short* hd = reinterpret_cast<const unsigned short*>(rg.rec(slot));
         ks = hd[lane]; ke = hd[lane + 1];
         sv += hd[33];                                  // the vals span starts at s & ~1
-        sb = rg.rec(slot) + kRecHdr + lane;
+        sw = reinterpret_cast<const unsigned*>(rg.rec(slot) + kRecHdr) + lane;     // word g of this lane at sw[32 g]
+        gmax = rg.rec_words - 1;
     } else {
         const int* rp = rg.rp(slot);
         const int base = rp[0] & ~3;
@@ -416,6 +422,39 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
     }
     const int trips = __reduce_max_sync(0xffffffffu, (ke - ks + U - 1) / U);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    if constexpr (CMP && GF && !FOLD) {
+        // Streamlined trip for the common case: every row of the tile fits one trip and the tile is not
+        // the ragged last one.  The record pads short rows with the code of offset 0, so every
+        // padding gather reads x[row] (a valid address) and only the DFMA is predicated: ~10 instead
+        // of ~22 instructions per entry -- the pinned kernel is bound by instruction issue
+        // (ncu: 21 k warp instructions per SM and iteration through 4 schedulers in ~8 k cycles).
+        if (trips == 1 && row - lane + (kTileRows - 1) < rg.n) {
+            constexpr int NW = (U + 3) / 4;
+            unsigned cw[NW];
+#pragma unroll
+            for (int g = 0; g < NW; ++g) cw[g] = sw[32 * (g < gmax ? g : gmax)];
+            double xv[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const unsigned code = __byte_perm(cw[u >> 2], 0u, 0x4440u | (unsigned)(u & 3));
+                xv[u] = ld_global_f64(x + (row + rg.offtab[code]));
+            }
+            const double* sr = sv + ks;
+            const int len = ke - ks;
+#pragma unroll
+            for (int u = 0; u < U; u += 3) {
+                const double v0 = sr[u], v1 = sr[u + 1], v2 = sr[u + 2];
+                if (u < len)     a0 = fma(v0, xv[u], a0);
+                if (u + 1 < len) a1 = fma(v1, xv[u + 1], a1);
+                if (u + 2 < len) a2 = fma(v2, xv[u + 2], a2);
+            }
+            if (!pinned) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&rg.empty[slot]);
+            }
+            return (a0 + a1) + a2;
+        }
+    }
     if (trips == 0 && !pinned) {
         __syncwarp();
         if (lane == 0) mbar_arrive(&rg.empty[slot]);
@@ -424,13 +463,29 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
         const int k = ks + t * U;
         int c[U];
         double v[GF ? 1 : U], xv[U];
+        // compressed index: the trip's U codes sit in (U + 6) / 4 consecutive 32-bit words of this
+        // lane (four codes per word); entry u is byte (t U mod 4) + (u mod 4) of the word pair
+        // {u / 4, u / 4 + 1}: one PRMT each, and 4 (U = 9) or 8 (U = 27) conflict-free loads per trip
+        constexpr int NW = CMP ? (U + 6) / 4 : 1;
+        unsigned cw[NW];
+        unsigned cbase = 0;
+        if constexpr (CMP) {
+            const int g0 = (t * U) >> 2;
+            cbase = (unsigned)(t * U) & 3u;
+#pragma unroll
+            for (int g = 0; g < NW; ++g) cw[g] = sw[32 * (g0 + g < gmax ? g0 + g : gmax)];
+        }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const bool in = k + u < ke;
             const int kk = in ? k + u : 0;
             int cc;
-            if constexpr (CMP) cc = row + rg.offtab[sb[in ? (t * U + u) * 32 : 0]];
-            else               cc = sc[kk];
+            if constexpr (CMP) {
+                const unsigned code = __byte_perm(cw[u >> 2], cw[(u >> 2) + 1 < NW ? (u >> 2) + 1 : NW - 1], cbase + (u & 3)) & 0xffu;
+                cc = row + rg.offtab[in ? code : 0];
+            } else {
+                cc = sc[kk];
+            }
             c[u] = in ? cc : 0;
             if constexpr (!GF) { const double vv = sv[kk]; v[u] = in ? vv : 0.0; }
         }

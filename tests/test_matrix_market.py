@@ -87,12 +87,12 @@ def test_loaded_matrix_through_cg_solve():
     from oracle import cg_oracle as orc
     n, rp, ci, va = read_matrix_market(FIXTURE)
     b = gi.seeded_vector(11, n)
-    ref = orc.cg(rp, ci, va, b, rtol=1e-12, maxit=n)
+    ref = orc.cg(rp, ci, va, b, rtol=1e-8, maxit=n)     # (a 64-row system: below ~1e-10 its residual norms are rounding noise)
     A = cg.CG(*(torch.from_numpy(a).cuda() for a in (rp, ci, va)))
     assert A.check_csr()
     for loop in (0, 1):
         A.set_option("loop", loop)
-        x, res = A.solve(torch.from_numpy(b).cuda(), rtol=1e-12, maxit=n)
+        x, res = A.solve(torch.from_numpy(b).cuda(), rtol=1e-8, maxit=n)
         assert res.status == 0 and abs(res.iters - ref.iters) <= 1
         k = min(50, ref.iters, res.iters)
         h = res.hist.cpu().numpy()

@@ -126,7 +126,7 @@ def test_two_rank_halo_exchange_and_recurrence_gloo(tmp_path):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg,grid", [(0, None), (4, 24)])
+@pytest.mark.parametrize("cfg,grid", [(0, None), (2, 20)])
 def test_rowblock_cg_single_rank_on_gpu(cfg, grid):
     """RowBlockCG with one rank (no peers: the halo is empty) runs the same recurrence through
     cg_spmv with device-side scalars and a host look every 16 iterations: all four bands against the
