@@ -364,6 +364,7 @@ def main():
     ap.add_argument("--fold", type=int, default=None)
     ap.add_argument("--pin", type=int, default=None)
     ap.add_argument("--compress", type=int, default=None)
+    ap.add_argument("--algo", type=int, default=None, help="with --profile: 1 = Chronopoulos-Gear, 2 = pipelined CG")
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -428,6 +429,8 @@ def main():
             Ap.set_option("pin", args.pin)
         if args.compress is not None:
             Ap.set_option("compress", args.compress)
+        if args.algo is not None:
+            Ap.set_option("algo", args.algo)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []
@@ -445,7 +448,7 @@ def main():
         rec = {"profile_config": args.profile, "iters": args.profile_iters, "us_per_iteration": out,
                "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid"),
                "compressed": Ap.info("compressed"), "pinned_tiles": Ap.info("pinned_tiles"),
-               "ring_slots": Ap.info("ring_slots"), "fold": Ap.info("fold"), "resident_rows": Ap.info("resident_rows")}
+               "ring_slots": Ap.info("ring_slots"), "fold": Ap.info("fold"), "resident_rows": Ap.info("resident_rows"), "algo": Ap.info("algo")}
         if tr is not None:
             # [cta, iter, slot] clock64 stamps -> cycles per interval; skip the first 2 iterations
             full = tr.cpu().numpy().astype(np.int64)
@@ -540,6 +543,8 @@ def main():
     # 2 GiB sweeps come from HBM
     l2_gbs = A.probe_read_bandwidth(40 << 20, reps=50)
     hbm_read_gbs = A.probe_read_bandwidth(2 << 30, reps=5)
+    sync_probe = {name: A.probe_grid_sync(kind, 3000) for kind, name in
+                  ((0, "counter_barrier"), (1, "relaxed_allreduce_x2_plus_counter_barrier_mean"), (2, "fenced_allreduce"))}
     t_iter = t_dev / iters_total if world == 1 else None
     launch2 = describe(A)
     kernel2 = kernel_name(A)
@@ -582,6 +587,8 @@ def main():
                         "hbm_read_gbs_measured_here": hbm_read_gbs,
                         "us_per_iteration": t_iter * 1e6 if t_iter else None,
                         "us_at_l2_peak": bytes_it / l2_gbs / 1e3, "us_at_hbm_peak": bytes_it / peak / 1e3},
+        "grid_sync_probe_cycles": {**sync_probe, "what": "cg_probe_grid_sync: mean cycles per synchronisation, 148 CTAs, "
+                                   "back to back with nothing in between (the floor; inside a solve they also absorb the CTAs' skew)"},
         "paper_context": {"source": "PAPER.md:52-57 Table I (Tesla T10 / Core 2 Duo, the paper's own FEM matrix)",
                           "opencl_1gpu_iters_per_s": 116 / 0.659, "matlab_pcg_iters_per_s": 117 / 3.17,
                           "opencl_4gpu_iters_per_s": 116 / 0.380, "opencl_1gpu_gflops": 1.45, "matlab_gflops": 0.303},

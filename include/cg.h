@@ -177,8 +177,14 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               (SURVEY.md 8(f) rank 2): w = A r, ONE all-reduce of (r.r, w.r) and one barrier
  *               that publishes r per iteration; same iterates in exact arithmetic, different
  *               rounding (held to the same parity bands in the tests, never the default).
- *               Applies to loop 0 with the vectors in registers and no preconditioner;
- *               otherwise the textbook path runs (cg_get_info "algo" tells which).
+ *               2 = pipelined CG (Ghysels-Vanroose): w = A r, q = A w, ONE counter barrier per
+ *               iteration; the partial sums of (r.r, w.r) are published by that barrier and read
+ *               back after the SpMV, so the reduction needs no synchronisation of its own.  One
+ *               more recurrence than 1 (more rounding); same status as 1.
+ *               Both apply to loop 0 with the vectors in registers and no preconditioner (2 also
+ *               needs kernel shape 3 or 4); otherwise the textbook path runs (cg_get_info "algo"
+ *               tells which).  With 2 the SpMV of the next iteration is started before the stop
+ *               test of the current one is known; iters still counts the updates of x.
  *   "compress"  1 (default) = use the compressed index once cg_compress_index has built it;
  *               0 = plain CSR slots
  *   "ring_slots" cap on the ring depth (8..64)
@@ -211,6 +217,16 @@ int cg_get_info(cg_handle* h, const char* name, int64_t* value);
  * bandwidth.  Synchronises the stream. */
 int cg_probe_read_bandwidth(cg_handle* h, const void* d_buf, size_t bytes, int reps,
                             double* h_gbs, void* cuda_stream);
+
+/* Grid-synchronisation probe (a profiling aid for DESIGN.md's latency figures): runs `reps`
+ * synchronisations of one kind on the solve's own grid (one CTA of 512 threads per SM,
+ * cooperative launch) with the very device functions cg_solve uses, and returns the mean cycles
+ * per synchronisation over all CTAs in *h_cycles.  kind 0 = counter barrier (no payload; what
+ * follows K3), 1 = push/poll all-reduce carrying only its payload (after K1 and K2; every third
+ * one is replaced by a counter barrier, as the slot-recycling rule demands, so the figure is the
+ * mean of two all-reduces and one barrier), 2 = all-reduce fenced on both sides (prologue, folded
+ * loop).  Synchronises the stream.  CG_ETIMEOUT if the watchdog tripped. */
+int cg_probe_grid_sync(cg_handle* h, int kind, int reps, double* h_cycles, void* cuda_stream);
 
 /* Phase trace of the persistent loop (loop mode 0), a profiling aid: with a non-NULL
  * d_trace (device uint64[grid * (iters + 1) * 16], grid = cg_get_info "grid"), thread 0 of

@@ -36,6 +36,7 @@ SIGNATURES = {
     "cg_solve_host": (ctypes.c_int, [_vp, _vp, _vp, _f64, _i64, _vp, ctypes.POINTER(_i64),
                                      ctypes.POINTER(_f64), _vp, _sz, _vp]),
     "cg_probe_read_bandwidth": (ctypes.c_int, [_vp, _vp, _sz, ctypes.c_int, ctypes.POINTER(_f64), _vp]),
+    "cg_probe_grid_sync": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(_f64), _vp]),
     "cg_set_trace": (ctypes.c_int, [_vp, _vp, _i64]),
     "cg_set_option": (ctypes.c_int, [_vp, ctypes.c_char_p, _i64]),
     "cg_get_info": (ctypes.c_int, [_vp, ctypes.c_char_p, ctypes.POINTER(_i64)]),
@@ -171,6 +172,15 @@ def cg_probe_read_bandwidth(h: int, d_buf: int, nbytes: int, reps: int, stream: 
     return out.value
 
 
+def cg_probe_grid_sync(h: int, kind: int, reps: int, stream: int = 0) -> float:
+    """Mean cycles per grid synchronisation of `kind` (0 counter barrier, 1 relaxed all-reduce mix, 2 fenced)."""
+    out = _f64()
+    rc = lib().cg_probe_grid_sync(h, kind, reps, ctypes.byref(out), stream)
+    if rc != 0:
+        raise CGError(rc, "cg_probe_grid_sync")
+    return out.value
+
+
 def cg_set_trace(h: int, d_trace: Optional[int], iters: int) -> None:
     rc = lib().cg_set_trace(h, d_trace, iters)
     if rc != 0:
@@ -262,6 +272,9 @@ class CG:
         """GB/s of a read-only sweep over a scratch buffer of nbytes (L2 if it fits, else HBM)."""
         buf = self.torch.ones(nbytes // 4, dtype=self.torch.int32, device=self.device)
         return cg_probe_read_bandwidth(self.h, buf.data_ptr(), buf.numel() * 4, reps, self._stream())
+
+    def probe_grid_sync(self, kind: int, reps: int = 2000) -> float:
+        return cg_probe_grid_sync(self.h, kind, reps, self._stream())
 
     def check_csr(self) -> bool:
         return cg_check_csr(self.h, self._stream()) == 0

@@ -442,6 +442,7 @@ struct StreamFns {
     const void* k1[2]; const void* k2; const void* k3;
     const void* persistent[2][kNumPersistent];
     const void* cg1[2][2];                 // option "algo" = 1 (Chronopoulos-Gear): [cmp][R == 4]
+    const void* pipe[2][2];                // option "algo" = 2 (pipelined CG)
 };
 
 template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(StreamFns& f) {
@@ -459,6 +460,12 @@ template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(Stre
     f.persistent[c][kR4Fold]   = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, true, CMP>;
     f.cg1[c][0] = (const void*)cgs::ks_persistent_cg1<W, NP, U, GF, 2, CMP>;
     f.cg1[c][1] = (const void*)cgs::ks_persistent_cg1<W, NP, U, GF, 4, CMP>;
+    if constexpr (NP != 4) {               // the single- and no-reduction loops exist for shapes 3 and 4 only (build time)
+        f.pipe[c][0] = (const void*)cgs::ks_persistent_pipe<W, NP, U, GF, 2, CMP>;
+        f.pipe[c][1] = (const void*)cgs::ks_persistent_pipe<W, NP, U, GF, 4, CMP>;
+    } else {
+        f.pipe[c][0] = f.pipe[c][1] = nullptr;
+    }
 }
 template <int W, int NP, int U, bool GF> static StreamFns make_stream_fns() {
     StreamFns f;
@@ -664,10 +671,13 @@ static bool fold_effective(const cg_handle* h, int v, int precond, const Geo& g)
     return gathers <= 500.0;
 }
 
-// Option "algo" = 1 (Chronopoulos-Gear) applies to the persistent streamed kernel with the vectors
-// in registers and no preconditioner; everything else runs the textbook recurrence.
-static bool algo1_effective(const cg_handle* h, int v, int precond) {
-    return h->algo_opt == 1 && h->loop == 0 && !precond && resident_rows(h, v) > 0;
+// Options "algo" = 1 (Chronopoulos-Gear) and 2 (pipelined CG) apply to the persistent streamed
+// kernel with the vectors in registers and no preconditioner; everything else runs the textbook
+// recurrence.
+static int algo_effective(const cg_handle* h, int v, int precond) {
+    if (h->algo_opt == 0 || h->loop != 0 || precond || resident_rows(h, v) == 0) return 0;
+    if (h->algo_opt == 2 && stream_fns(v - 2).pipe[0][0] == nullptr) return 0;
+    return h->algo_opt;
 }
 
 static void fill_params(const cg_handle* h, Params* P, const double* b, double* x, double rtol,
@@ -785,8 +795,10 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
             for (const void* fn : two) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
             for (int k = 0; k < kNumPersistent; ++k)
                 CKH(cudaFuncSetAttribute(f.persistent[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
-            for (int k = 0; k < 2; ++k)
+            for (int k = 0; k < 2; ++k) {
                 CKH(cudaFuncSetAttribute(f.cg1[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
+                if (f.pipe[c][k]) CKH(cudaFuncSetAttribute(f.pipe[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
+            }
         }
     }
     *out = h;
@@ -888,7 +900,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         h->pin_opt = (int)value; drop_graph();
         return CG_OK;
     }
-    if (!strcmp(name, "algo")) { if (value < 0 || value > 1) return CG_EINVAL; h->algo_opt = (int)value; return CG_OK; }
+    if (!strcmp(name, "algo")) { if (value < 0 || value > 2) return CG_EINVAL; h->algo_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "smem_cap_kb")) { if (value < 0 || value > 227) return CG_EINVAL; h->smem_cap_kb = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
@@ -931,7 +943,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "slot_bytes")) *value = v >= 2 ? g.slot_bytes : 0;
     else if (!strcmp(name, "resident_rows")) *value = resident_rows(h, v);
     else if (!strcmp(name, "fold")) *value = fold_effective(h, v, 0, g) ? 1 : 0;
-    else if (!strcmp(name, "algo")) *value = algo1_effective(h, v, 0) ? 1 : 0;
+    else if (!strcmp(name, "algo")) *value = algo_effective(h, v, 0);
     else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
     else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
     else if (!strcmp(name, "from_hbm")) *value = g.from_hbm ? 1 : 0;
@@ -971,6 +983,36 @@ extern "C" int cg_probe_read_bandwidth(cg_handle* h, const void* d_buf, size_t b
     CK(cudaGetLastError());
     h->launches = reps + 1;
     *h_gbs = (double)(n16 * 16) * reps / ((double)ms * 1e-3) / 1e9;
+    return CG_OK;
+}
+
+extern "C" int cg_probe_grid_sync(cg_handle* h, int kind, int reps, double* h_cycles, void* cuda_stream) {
+    if (!h || !h_cycles || kind < 0 || kind > 2 || reps < 1 || reps > (1 << 20) || h->sms > cgs::kBarGrid) return CG_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    constexpr int W = 16;
+    const void* fn = (const void*)cgs::ks_probe_sync<W>;
+    Geo g; memset(&g, 0, sizeof(g));
+    g.slots = 1; g.slot_bytes = 128;
+    Params P;
+    fill_params(h, &P, nullptr, nullptr, 0.0, 0, nullptr, 0, 4, g);
+    unsigned long long* out = reinterpret_cast<unsigned long long*>(h->part1);       // kMaxGrid slots of scratch
+    CK(cudaMemsetAsync(&h->scal->bar, 0, sizeof(unsigned long long) + 2 * sizeof(int), st));     // bar, abort
+    CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));
+    void* args[] = {&P, &kind, &reps, &out};
+    const size_t smem = (size_t)g.slots * g.slot_bytes + cgs::kSmemTail;
+    CK(cudaLaunchCooperativeKernel(fn, dim3(h->sms), dim3(32 * W), args, smem, st));
+    unsigned long long* host = static_cast<unsigned long long*>(malloc(sizeof(unsigned long long) * (size_t)h->sms));
+    if (!host) return CG_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(host, out, sizeof(unsigned long long) * (size_t)h->sms, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    double sum = 0.0; bool dead = false;
+    for (int i = 0; i < h->sms; ++i) { sum += (double)host[i]; dead = dead || host[i] == 0; }
+    free(host);
+    CK(e);
+    h->launches = 1;
+    if (dead) return CG_ETIMEOUT;
+    // in kind 1 every third synchronisation is the counter barrier the recycling rule asks for
+    *h_cycles = sum / h->sms / reps;
     return CG_OK;
 }
 
@@ -1095,7 +1137,9 @@ static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol,
                            : R == 2 ? (precond ? kR2Jacobi : fold ? kR2Fold : kR2)
                                     : (precond ? kR4Jacobi : fold ? kR4Fold : kR4);
             h->last_resident = R; h->last_fold = fold ? 1 : 0;
-            const void* fn = algo1_effective(h, v, precond) ? f.cg1[g.cmp][R == 4 ? 1 : 0] : f.persistent[g.cmp][kind];
+            const int algo = algo_effective(h, v, precond);
+            const void* fn = algo == 1 ? f.cg1[g.cmp][R == 4 ? 1 : 0] : algo == 2 ? f.pipe[g.cmp][R == 4 ? 1 : 0]
+                                       : f.persistent[g.cmp][kind];
             CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));        // arm the all-reduce slots
             CK(cudaLaunchCooperativeKernel(fn, dim3(G), dim3(32 * (f.W + f.NP)), args, g.smem, st));
         }

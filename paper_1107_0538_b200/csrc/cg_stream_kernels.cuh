@@ -569,4 +569,241 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
     if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(gam); }
 }
 
+// ---- option "algo" = 2: pipelined conjugate gradients (Ghysels & Vanroose 2014), the form of the
+// iteration whose ONE reduction is hidden behind the SpMV.  With w = A r and q = A w:
+//     gamma = r.r ; delta = w.r                    (partials written BEFORE the barrier below)
+//     q = A w                                      (K1; the partials are read while it runs)
+//     beta = gamma / gamma_old ; alpha = gamma / (delta - beta gamma / alpha_old)
+//     z = q + beta z ; s = w + beta s ; p = r + beta p ; x += alpha p ; r -= alpha s ; w -= alpha z
+//     -- counter barrier: w and the partials are published --
+// One grid synchronisation per iteration: the counter barrier's release / acquire fences make
+// every CTA's partials (one plain store per CTA and value, double-buffered by iteration parity)
+// visible to everyone who leaves the barrier, so the "all-reduce" is 148 L2 reads per value that
+// every warp issues after its K1 tiles and sums in one fixed order: nobody polls, and the
+// reduction costs no grid synchronisation of its own.
+// Same iterates as the textbook recurrence in exact arithmetic; more recurrences,
+// hence more rounding: an OPTION, held to the same parity bands in the tests, never the default.
+// hist[k] = ||r_k||; k counts the updates of x (each pass also starts the SpMV of the next
+// one before it can know that the stop test is met: that one is the price of the overlap).
+template <int W>
+__device__ __forceinline__ bool grid_barrier_partials(const Params& P, const Ring& rg, unsigned long long& nbar, int G,
+                                                      int cta, int buf, double a, double b, double c) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+    if (lane == 0) { rg.red[warp] = a; rg.red[32 + warp] = b; rg.red[64 + warp] = c; }
+    consumer_sync<W>();                    // also: all phase stores of the CTA happen-before the fence below
+    if (warp == 0) {
+        a = warp_sum(lane < W ? rg.red[lane] : 0.0);
+        b = warp_sum(lane < W ? rg.red[32 + lane] : 0.0);
+        c = warp_sum(lane < W ? rg.red[64 + lane] : 0.0);
+        if (lane == 0) {
+            double* slot = P.part0 + (size_t)buf * 3 * kBarGrid + cta;
+            slot[0] = a; slot[kBarGrid] = b; slot[2 * kBarGrid] = c;
+            unsigned long long* ctr = &P.scal->bar;
+            asm volatile("fence.acq_rel.gpu;" ::: "memory");
+            asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(1ULL) : "memory");
+            const unsigned long long target = (++nbar) * (unsigned long long)G;
+            bounded_spin(rg, [&] { return ld_relaxed_u64(ctr) >= target; });
+            asm volatile("fence.acq_rel.gpu;" ::: "memory");
+            rg.red[kRedTot + kBarVals] = rg.ctl[4] != 0 ? 1.0 : 0.0;
+        }
+    }
+    consumer_sync<W>();
+    return rg.red[kRedTot + kBarVals] != 0.0;
+}
+
+// Every warp: start the reads of the G per-CTA partials of NV values (lane l takes CTAs l, l + 32, ...).
+template <int NV>
+__device__ __forceinline__ void partials_issue(const Params& P, int G, int buf, double (&u)[NV][kBarM]) {
+    const int lane = threadIdx.x & 31;
+    const double* base = P.part0 + (size_t)buf * 3 * kBarGrid;
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+#pragma unroll
+        for (int m = 0; m < kBarM; ++m) {
+            const int j = lane + 32 * m;
+            u[i][m] = j < G ? __longlong_as_double((long long)ld_relaxed_u64(reinterpret_cast<const unsigned long long*>(base + i * kBarGrid + j))) : 0.0;
+        }
+}
+template <int NV>
+__device__ __forceinline__ void partials_sum(const double (&u)[NV][kBarM], double (&tot)[NV]) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        double t = 0.0;
+#pragma unroll
+        for (int m = 0; m < kBarM; ++m) t += u[i][m];
+        tot[i] = warp_sum(t);              // xor tree: the same bits in every lane, warp and CTA
+    }
+}
+
+template <int W, int NP, int U, bool GF, int R, bool CMP>
+__global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_pipe(Params P) {
+    static_assert(R > 0, "vectors in registers");
+    CGS_PROLOGUE(W);
+    ring_init(P, rg);
+    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, LLONG_MAX, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
+    const int lane = threadIdx.x & 31;
+    const bool lead = cta == 0 && threadIdx.x == 0;
+    Scal* S = P.scal;
+    unsigned long long nbar = 0;
+    unsigned long long pass = 0;
+    RingPos pos{0u, 0u, 0u};
+    double xr[R], rv[R], pv[R], sv[R], wv[R], zv[R];
+    long long row[R];
+    // two published vectors, used alternately: pass k gathers w_k from one and stores w_{k+1} into the
+    // other, so a CTA that is ahead never overwrites what a CTA still in its K1 is gathering (there is
+    // no synchronisation between K1 and the update here, unlike the other loops)
+    double* const wpub[2] = {P.p, P.q};
+
+    // prologue: r0 = b - A x0 (published), w0 = A r0 (published with the partials of gamma0, delta0, b.b)
+    double abb = 0.0;
+    consumers_begin_pass(rg, pass);
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        const long long i = (tb + j) * kTileRows + lane;
+        row[kk] = (j < Tc && i < P.n) ? i : -1;
+        xr[kk] = 0.0; pv[kk] = 0.0; sv[kk] = 0.0; wv[kk] = 0.0; zv[kk] = 0.0;
+        double bi = 0.0;
+        if (row[kk] >= 0) { xr[kk] = P.x[i]; bi = P.b[i]; }
+        rv[kk] = bi;
+    }
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        double q = 0.0;
+        if (j < Tc) q = consume_tile<U, false, CMP, GF>(rg, P.x, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+        if (row[kk] >= 0) {
+            abb = fma(rv[kk], rv[kk], abb);
+            rv[kk] = rv[kk] - q;
+            wpub[0][row[kk]] = rv[kk];
+        }
+    }
+    ++pass; pos = ring_next_pass(rg, pos, Tc);
+    bool dead = grid_barrier_partials<W>(P, rg, nbar, G, cta, 0, 0.0, 0.0, abb);            // r0 and b.b are published
+    double agam = 0.0, adel = 0.0;
+    consumers_begin_pass(rg, pass);
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        if (j < Tc) wv[kk] = consume_tile<U, false, CMP, GF>(rg, wpub[0], pos, j, lane, (int)((tb + j) * kTileRows + lane));
+        if (row[kk] >= 0) { agam = fma(rv[kk], rv[kk], agam); adel = fma(wv[kk], rv[kk], adel); wpub[1][row[kk]] = wv[kk]; }
+    }
+    ++pass; pos = ring_next_pass(rg, pos, Tc);
+    double bb;
+    {
+        double u[1][kBarM], t[1];
+        const double* base = P.part0 + 2 * kBarGrid;                                            // value 2 of buffer 0
+#pragma unroll
+        for (int m = 0; m < kBarM; ++m) { const int j = lane + 32 * m; u[0][m] = j < G ? __ldcg(base + j) : 0.0; }
+        partials_sum<1>(u, t);
+        bb = t[0];
+    }
+    dead = grid_barrier_partials<W>(P, rg, nbar, G, cta, 1, agam, adel, 0.0) || dead;     // w0 and (gamma0, delta0) are published
+    int buf = 1;                               // parity of the published vector AND of the partials this pass reads
+
+    long long k = 0; int stop = 0, status = CG_OK;
+    double gam = 0.0, gam_old = 1.0, alpha = 1.0, thresh = P.rtol * sqrt(bb);
+    if (dead) { stop = 1; status = CG_ETIMEOUT; }
+    unsigned long long* tr = (P.trace && threadIdx.x == 0)
+        ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
+#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
+    while (!stop) {
+        CGS_STAMP(k, 0);
+        // K1: q = A w
+        double qv[R];
+        consumers_begin_pass(rg, pass);
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            const int j = warp + kk * W;
+            qv[kk] = 0.0;
+            if (j < Tc) qv[kk] = consume_tile<U, false, CMP, GF>(rg, wpub[buf], pos, j, lane, (int)((tb + j) * kTileRows + lane));
+        }
+        ++pass; pos = ring_next_pass(rg, pos, Tc);
+        CGS_STAMP(k, 1);
+        // the reduction: every warp reads the 148 x 2 partials (published by the barrier that ended the
+        // previous pass) and sums them in the one fixed order.  Issuing these reads before K1 hides their
+        // L2 round trip but holds 20 registers through K1, which then spills (measured: K1 9.4 k against
+        // 6.9 k cycles); here they cost one exposed round trip and no CTA barrier.
+        double u[2][kBarM];
+        partials_issue<2>(P, G, buf, u);
+        double t2[2];
+        partials_sum<2>(u, t2);
+        gam = t2[0];
+        const double del = t2[1];
+        CGS_STAMP(k, 2);
+        // continue-condition on ||r_k|| (k = 0: the test "before the first iteration")
+        if (bb == 0.0) {
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) xr[kk] = 0.0;
+            gam = 0.0;
+        }
+        const double res = sqrt(gam);
+        if (lead && P.hist) P.hist[k] = res;
+        if (bb == 0.0 || res <= thresh) { stop = 1; status = CG_OK; break; }
+        if (k >= P.maxit) { stop = 1; status = CG_MAXIT; break; }
+        const double beta = k > 0 ? gam / gam_old : 0.0;
+        const double denom = k > 0 ? del - beta * gam / alpha : del;         // = p.A p of the direction about to be used
+        if (!(denom > 0.0) || !finite_d(denom)) { stop = 1; status = CG_BREAKDOWN; break; }
+        alpha = gam / denom;
+        gam_old = gam;
+        CGS_STAMP(k, 3); CGS_STAMP(k, 4); CGS_STAMP(k, 5);
+        // vector recurrences, registers only; partials of the next gamma, delta
+        const double na = -alpha;
+        agam = 0.0; adel = 0.0;
+#pragma unroll
+        for (int kk = 0; kk < R; ++kk) {
+            if (row[kk] < 0) continue;
+            zv[kk] = fma(beta, zv[kk], qv[kk]);
+            sv[kk] = fma(beta, sv[kk], wv[kk]);
+            pv[kk] = fma(beta, pv[kk], rv[kk]);
+            xr[kk] = fma(alpha, pv[kk], xr[kk]);
+            rv[kk] = fma(na, sv[kk], rv[kk]);
+            wv[kk] = fma(na, zv[kk], wv[kk]);
+            wpub[buf ^ 1][row[kk]] = wv[kk];
+            agam = fma(rv[kk], rv[kk], agam);
+            adel = fma(wv[kk], rv[kk], adel);
+        }
+        k += 1;
+        CGS_STAMP(k - 1, 6);
+        buf ^= 1;
+        dead = grid_barrier_partials<W>(P, rg, nbar, G, cta, buf, agam, adel, 0.0);        // the one synchronisation
+        CGS_STAMP(k - 1, 7);
+        if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
+    }
+#undef CGS_STAMP
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk)
+        if (row[kk] >= 0) P.x[row[kk]] = xr[kk];
+    if (threadIdx.x == 0) consumers_stop(rg, pass);
+    if (lead) { S->out_iters = k; S->out_status = status; S->out_res = sqrt(gam); }
+}
+
+// ---- cg_probe_grid_sync: the cost of the grid synchronisations themselves, measured with the very
+// device functions the solve uses, on the solve's grid (one CTA per SM, cooperative launch).
+// kind 0 = counter barrier, 1 = push/poll all-reduce carrying its payload only, 2 = fenced.
+// Thread 0 of every CTA writes the cycles of its `reps` synchronisations to out[cta].
+template <int W>
+__global__ void __launch_bounds__(32 * W, 1) ks_probe_sync(Params P, int kind, int reps, unsigned long long* out) {
+    CGS_PROLOGUE(W);
+    ring_init(P, rg);
+    unsigned bcount = 0;
+    unsigned long long nbar = 0;
+    double v[1] = {(double)threadIdx.x};
+    // one fenced all-reduce first: every CTA is resident and past its set-up before the clock starts
+    grid_allreduce<W, 1, true>(P, rg, bcount, cta, G, v);
+    const long long t0 = clock64();
+    bool dead = false;
+    for (int i = 0; i < reps && !dead; ++i) {
+        if (kind == 0) dead = grid_barrier_counter<W>(P, rg, nbar, G);
+        else if (kind == 1) {
+            // a relaxed all-reduce needs a fenced synchronisation within every window of three
+            dead = (i % 3 == 2) ? grid_barrier_counter<W>(P, rg, nbar, G) : grid_allreduce<W, 1, false>(P, rg, bcount, cta, G, v);
+        } else dead = grid_allreduce<W, 1, true>(P, rg, bcount, cta, G, v);
+    }
+    if (threadIdx.x == 0) out[cta] = dead ? 0ULL : (unsigned long long)(clock64() - t0);
+    (void)tb; (void)Tc;
+}
+
 }  // namespace cgs

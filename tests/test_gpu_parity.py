@@ -332,6 +332,10 @@ def test_phase_trace_and_bandwidth_probe(bound, cgmod):
     B.cg.set_option("pin", 1)
     gbs = B.cg.probe_read_bandwidth(32 << 20, reps=10)
     assert 500.0 < gbs < 50000.0
+    cyc = [B.cg.probe_grid_sync(kind, 500) for kind in (0, 1, 2)]
+    assert all(300.0 < c < 50000.0 for c in cyc) and cyc[2] > cyc[0]       # the fenced all-reduce costs more than the bare barrier
+    x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)                   # the probe leaves the handle usable
+    assert res.status == 0
     with pytest.raises(cgmod.CGError):
         cgmod.cg_probe_read_bandwidth(B.cg.h, 0, 1 << 20, 1, 0)
 
@@ -565,16 +569,18 @@ def test_generic_ctas_per_sm(bound, orc, ctas):
 # ---------------------------------------------------------------- single-reduction CG (8(f) rank 2, second half)
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
-def test_single_reduction_cg_parity(bound, orc, cfg):
-    """Option "algo" = 1: Chronopoulos-Gear CG (one all-reduce + one publish barrier per iteration).
-    Same Krylov iteration, different rounding: it must pass the same four bands against the same
+@pytest.mark.parametrize("algo", [1, 2])
+def test_single_reduction_cg_parity(bound, orc, cfg, algo):
+    """Option "algo" = 1: Chronopoulos-Gear CG (one all-reduce + one publish barrier per iteration);
+    "algo" = 2: pipelined CG (one barrier per iteration, the reduction hidden behind the SpMV).
+    Same Krylov iteration, different rounding: each must pass the same four bands against the same
     (unchanged) oracle as the textbook path, and return an x whose true residual, computed with the
     oracle's SpMV, meets rtol."""
     B = bound(cfg)
     p = B.p
     B.cg.set_option("loop", 0)
-    B.cg.set_option("algo", 1)
-    assert B.cg.info("algo") == 1
+    B.cg.set_option("algo", algo)
+    assert B.cg.info("algo") == algo
     ref = oracle_solve(orc, p, ("cg", cfg))
     x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
     check_solve_parity(res, x, ref)
@@ -595,12 +601,15 @@ def test_single_reduction_cg_parity(bound, orc, cfg):
     B.cg.set_option("algo", 0)
 
 
-def test_single_reduction_cg_breakdown(bound, cgmod):
+@pytest.mark.parametrize("algo", [1, 2])
+def test_single_reduction_cg_breakdown(bound, cgmod, algo):
     B = bound(0)
     neg = cgmod.CG(dev(B.p.rowptr), dev(B.p.colind), dev(-B.p.vals))
-    neg.set_option("algo", 1)
+    neg.set_option("algo", algo)
     x, res = neg.solve(B.b, rtol=1e-10, maxit=10)
     assert res.status == 2 and res.iters == 0
+    x, res = neg.solve(B.b, rtol=1e-10, maxit=0)
+    assert res.status == 1 and res.iters == 0
     neg.close()
 
 
