@@ -252,6 +252,22 @@ def per_config_leg(cg, torch, dev, cfg, p, args, peak, l2_gbs, flush_l2, with_cp
                              "spmv_gflops": 2 * p.nnz / t_k1 / 1e9,
                              "grid_sync_share_of_iteration": sync / it_cyc,
                              "what": "cg_set_trace over 24 iterations: K1 of the slowest CTA per iteration, scaled to the untraced iteration time"}
+    if cfg != 4 and A.info("loop") == 0:
+        # the reduced-synchronisation recurrences, reported BESIDE the textbook path (options, never the
+        # metric).  Timed on the solve to convergence: past the accuracy the arithmetic can reach their
+        # denominators lose positivity (CG_BREAKDOWN), so a fixed 2000 iterations is not a workload for them.
+        var = {}
+        for algo, name in ((1, "chronopoulos_gear"), (2, "pipelined")):
+            A.set_option("algo", algo)
+            if A.info("algo") == algo:
+                timed_solve(p.rtol, p.maxit, True)
+                runs = sorted((timed_solve(p.rtol, p.maxit, True) for _ in range(3)), key=lambda r: r[0])
+                t, it, st = runs[1]
+                var[name] = {"iterations": it, "status": st, "us_per_iteration": t / max(it, 1) * 1e6,
+                             "frac_of_hbm_roofline": bytes_it * it / t / 1e9 / peak,
+                             "what": "solve to convergence, prologue (two SpMVs) included"}
+        A.set_option("algo", 0)
+        rec["reduced_sync_variants"] = var
     if cfg != 4:
         timed_solve(p.rtol, p.maxit, True)
         tc = [timed_solve(p.rtol, p.maxit, True) for _ in range(3)]
@@ -456,7 +472,9 @@ def main():
             rec["ring_stats"] = {"producer_wait_cycles": float(st[:, 0].mean()), "producer_total_cycles": float(st[:, 1].mean()),
                                  "tiles_issued": float(st[:, 2].mean()), "consumer_warp0_full_wait_cycles": float(st[:, 3].mean())}
             t = full[:, 2:args.profile_iters - 1, :]
-            names = ["K1 work", "barrier 1", "alpha + K2 work", "barrier 2", "beta", "K3 work", "barrier 3"]
+            names = {0: ["K1 work", "barrier 1", "alpha + K2 work", "barrier 2", "beta", "K3 work", "barrier 3"],
+                     1: ["vector updates", "publish barrier", "K1 work", "all-reduce", "scalars", "(unused a)", "(unused b)"],
+                     2: ["K1 work", "partials read + sum", "scalars", "(unused a)", "(unused b)", "vector updates", "barrier"]}[Ap.info("algo")]
             d = np.diff(t[:, :, :8], axis=2)
             if t.shape[2] >= 16 and t[:, :, 8:].any():
                 dd = np.diff(t[:, :, 8:], axis=2)

@@ -511,8 +511,9 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
         ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
 #define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
     while (!stop) {
-        // trace slots keep the textbook kernel's meaning as far as it goes: 0 start, 1 K1 done, 2 past the
-        // all-reduce, 3..5 scalars, 6 vector updates done, 7 past the publish barrier of the NEXT K1's operand
+        // trace slots of this loop, in order: 0 pass start, 1 vector updates done, 2 past the publish
+        // barrier, 3 K1 done, 4 past the all-reduce, 5 = 6 = 7 scalars done
+        CGS_STAMP(k, 0);
         // vector updates (the textbook's K3 and K2 in one pass over the registers)
         const double na = -alpha;
 #pragma unroll
@@ -524,13 +525,12 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
             rv[kk] = fma(na, sv[kk], rv[kk]);
             rpub[row[kk]] = rv[kk];
         }
-        CGS_STAMP(k, 6);
+        CGS_STAMP(k, 1);
         dead = iter_sync<W, Plan, 0>(P, rg, bcount, nbar, cta, G, none,               // publishes r
                                      (tr && k < P.trace_iters) ? tr + k * kTraceSlots + 8 : nullptr);
-        CGS_STAMP(k, 7);
+        CGS_STAMP(k, 2);
         if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
         // K1: w = A r, partials of gamma' = r.r and delta = w.r
-        CGS_STAMP(k, 0);
         agam = 0.0; adel = 0.0;
         consumers_begin_pass(rg, pass);
 #pragma unroll
@@ -542,10 +542,10 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
             }
         }
         ++pass; pos = ring_next_pass(rg, pos, Tc);
-        CGS_STAMP(k, 1);
+        CGS_STAMP(k, 3);
         double v2[2] = {agam, adel};
         dead = iter_sync<W, Plan, 1>(P, rg, bcount, nbar, cta, G, v2);
-        CGS_STAMP(k, 2);
+        CGS_STAMP(k, 4);
         if (dead) { stop = 1; status = CG_ETIMEOUT; break; }
         const double gam_new = v2[0];
         del = v2[1];
@@ -559,7 +559,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
         gam = gam_new;
         if (!(denom > 0.0) || !finite_d(denom)) { stop = 1; status = CG_BREAKDOWN; break; }
         alpha = gam / denom;
-        CGS_STAMP(k - 1, 5);
+        CGS_STAMP(k - 1, 5); CGS_STAMP(k - 1, 6); CGS_STAMP(k - 1, 7);
     }
 #undef CGS_STAMP
 #pragma unroll
