@@ -196,6 +196,11 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               started (default unlimited: the ring is refilled across the grid barriers)
  *   "tpr", "ctas_per_sm"  lanes per row and CTAs per SM of the generic variant
  *   "values_changed" (any value) the caller rewrote vals: cached D^-1 is dropped
+ *   "checked"   1 = cg_spmv runs its checked twin: every index it forms (source ranges of the
+ *               bulk copies, offsets inside a slot, index codes, gathered columns) is validated
+ *               on the device before use and clamped when wrong; the call then synchronises and
+ *               returns CG_ECUDA ("... out-of-range indices caught") if any was.  The library's
+ *               own memcheck (compute-sanitizer is not available everywhere); default 0
  *   "spin_budget_ms" how long any device-side spin may last before the watchdog trips and
  *               the solve returns CG_ETIMEOUT (default 2000)
  *   "inject_fault" tests only: k > 0 makes producer warp 0 of CTA 0 announce its k-th tile
@@ -203,7 +208,8 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
  * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "pinned_tiles", "slot_bytes",
- * "resident_rows", "fold", "algo", "compressed", "index_codes", "from_hbm", "lines_per_gather_x100"
+ * "resident_rows", "fold", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
+ * counted by the last checked cg_spmv), "lines_per_gather_x100"
  * (cg_create statistic: 128-byte lines one warp-wide gather touches on average, times 100).
  * Unknown names return CG_EINVAL. */
 int cg_set_option(cg_handle* h, const char* name, int64_t value);

@@ -438,6 +438,7 @@ enum PersistentKind { kR0, kR0Jacobi, kR2, kR2Jacobi, kR2Fold, kR4, kR4Jacobi, k
 struct StreamFns {
     int W, NP, U;
     const void* spmv[2];
+    const void* spmv_checked[2];           // option "checked"
     const void* init_spmv[2]; const void* init_residual; const void* init_scalars;
     const void* k1[2]; const void* k2; const void* k3;
     const void* persistent[2][kNumPersistent];
@@ -448,6 +449,7 @@ struct StreamFns {
 template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(StreamFns& f) {
     constexpr int c = CMP ? 1 : 0;
     f.spmv[c] = (const void*)cgs::ks_spmv<W, NP, U, GF, CMP>;
+    f.spmv_checked[c] = (const void*)cgs::ks_spmv<W, NP, U, GF, CMP, true>;
     f.init_spmv[c] = (const void*)cgs::ks_init_spmv<W, NP, U, GF, CMP>;
     f.k1[c] = (const void*)cgs::ks1_spmv_dot<W, NP, U, GF, CMP>;
     f.persistent[c][kR0]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 0, false, false, CMP>;
@@ -508,7 +510,7 @@ struct cg_handle {
     int sms, smem_optin, clock_khz;
     size_t l2_bytes;
     int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, pin_opt, compress_opt;
-    int spin_budget_ms, inject_fault, algo_opt;
+    int spin_budget_ms, inject_fault, algo_opt, checked_opt;
     int max_row_len, max_tile_nnz, tpr;
     double lines_per_gather;               // cg_create statistic (k_gather_stats)
     int smem_cap_kb;                       // option: 0 = auto
@@ -520,6 +522,7 @@ struct cg_handle {
     unsigned long long* trace; int trace_iters;
     long long launches;
     int last_resident, last_fold;          // what the last persistent solve used (info)
+    int last_chk_errors;                   // violations counted by the last checked cg_spmv
 };
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -791,7 +794,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
         const void* one[] = {f.init_residual, f.init_scalars, f.k2, f.k3};
         for (const void* fn : one) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
         for (int c = 0; c < 2; ++c) {
-            const void* two[] = {f.spmv[c], f.init_spmv[c], f.k1[c]};
+            const void* two[] = {f.spmv[c], f.spmv_checked[c], f.init_spmv[c], f.k1[c]};
             for (const void* fn : two) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
             for (int k = 0; k < kNumPersistent; ++k)
                 CKH(cudaFuncSetAttribute(f.persistent[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
@@ -900,6 +903,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
         h->pin_opt = (int)value; drop_graph();
         return CG_OK;
     }
+    if (!strcmp(name, "checked")) { if (value < 0 || value > 1) return CG_EINVAL; h->checked_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "algo")) { if (value < 0 || value > 2) return CG_EINVAL; h->algo_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "smem_cap_kb")) { if (value < 0 || value > 227) return CG_EINVAL; h->smem_cap_kb = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
@@ -947,6 +951,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
     else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
     else if (!strcmp(name, "from_hbm")) *value = g.from_hbm ? 1 : 0;
+    else if (!strcmp(name, "check_errors")) *value = h->last_chk_errors;
     else if (!strcmp(name, "lines_per_gather_x100")) *value = (int64_t)(h->lines_per_gather * 100.0 + 0.5);
     else return CG_EINVAL;
     return CG_OK;
@@ -1040,6 +1045,22 @@ extern "C" int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_
     } else {
         const StreamFns& f = stream_fns(v - 2);
         void* args[] = {&P, &d_x, &d_y};
+        if (h->checked_opt) {
+            // the library's own memcheck: every index validated and clamped on the device, violations
+            // counted; this call synchronises and reports them
+            CK(cudaMemsetAsync(&h->scal->chk_errors, 0, sizeof(int), st));
+            CK(cudaLaunchKernel(f.spmv_checked[g.cmp], dim3(h->sms), dim3(32 * (f.W + f.NP)), args, g.smem, st));
+            CK(cudaMemcpyAsync(h->h_scal, h->scal, sizeof(Scal), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            h->launches = 1;
+            h->last_chk_errors = h->h_scal->chk_errors;
+            if (h->h_scal->chk_errors) {
+                snprintf(g_cuda_err, sizeof(g_cuda_err), "checked cg_spmv: %d out-of-range indices caught and clamped (corrupt CSR arrays?)",
+                         h->h_scal->chk_errors);
+                return CG_ECUDA;
+            }
+            return CG_OK;
+        }
         CK(cudaLaunchKernel(f.spmv[g.cmp], dim3(h->sms), dim3(32 * (f.W + f.NP)), args, g.smem, st));
     }
     CK(cudaGetLastError());

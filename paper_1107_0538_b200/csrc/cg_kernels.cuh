@@ -44,7 +44,7 @@ struct Scal {             // device-resident scalar state, zeroed before each so
     int brk[2];           // breakdown seen by K2 of this parity
     unsigned long long bar;       // grid barrier arrival counter
     int abort;            // a device-side spin ran out of its budget (watchdog): the results are void
-    int pad0;
+    int chk_errors;       // option "checked": index violations caught (and clamped) by a checked cg_spmv
     long long out_iters;  // result block, copied to the host at the end
     long long out_status;
     double out_res;

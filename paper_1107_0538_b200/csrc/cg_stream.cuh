@@ -80,6 +80,7 @@ struct Ring {
     int P, Q;                         // pinned slots [0, P) and streaming slots [P, P + Q), P + Q <= S
     int rec_words;                    // compressed index: 32-bit code words per lane in a record
     int n;                            // rows of the matrix
+    int ncodes;                       // entries of the offset table in shared memory
     long long budget;                 // cycles a spin may last
     Scal* scal;
     unsigned long long* acc;          // optional: cycles this thread waited on full barriers (trace)
@@ -100,7 +101,7 @@ struct Ring {
 __device__ __forceinline__ Ring ring_view(const Params& P, unsigned char* dyn) {
     Ring rg;
     rg.S = P.slots; rg.slot_bytes = P.slot_bytes; rg.cap = P.cap; rg.acc = nullptr;
-    rg.P = P.pinned; rg.Q = P.stream_slots; rg.rec_words = (P.rec_stride - kRecHdr) / 128; rg.n = (int)P.n;
+    rg.P = P.pinned; rg.Q = P.stream_slots; rg.rec_words = (P.rec_stride - kRecHdr) / 128; rg.n = (int)P.n; rg.ncodes = P.ncodes_smem;
     rg.budget = P.spin_budget; rg.scal = P.scal;
     rg.slots = dyn;
     unsigned char* tail = dyn + (size_t)P.slots * P.slot_bytes;
@@ -164,10 +165,29 @@ __device__ __forceinline__ bool mbar_wait_bounded(const Ring& rg, uint64_t* bar,
 
 // ---------------------------------------------------------------- producer
 
-template <bool CMP>
+// CHK (option "checked", cg_spmv only): every index is validated before it is used -- source
+// ranges of the bulk copies against the arrays' lengths, slot offsets against the slot's size,
+// codes against the table, gathered columns against n -- violations are counted in
+// Scal::chk_errors and the access is clamped, so a checked run never touches memory it should not.
+// This is the library's own stand-in for compute-sanitizer's memcheck (closed on this pool).
+__device__ __forceinline__ void chk_fail(const Ring& rg) { atomicAdd(&rg.scal->chk_errors, 1); }
+
+template <bool CMP, bool CHK = false>
 __device__ __forceinline__ void producer_issue(const Params& P, const Ring& rg, int slot, long long t,
                                                int s, int e, uint64_t policy, unsigned tag, bool drop) {
     constexpr int A = CMP ? 1 : 3;                     // span alignment in entries (16 bytes of the narrowest array)
+    if constexpr (CHK) {
+        const long long ntiles = (P.n + kTileRows - 1) / kTileRows;
+        const int lo = s & ~A;
+        const bool bad = t < 0 || t >= ntiles || s < 0 || e < s || (long long)e > P.nnz || e - lo > rg.cap ||
+                         slot < 0 || slot >= rg.S;
+        if (bad) {                                     // announce nothing: complete the phase with a plain arrival
+            chk_fail(rg);
+            rg.tag[slot < 0 || slot >= rg.S ? 0 : slot] = tag;
+            mbar_arrive(&rg.full[slot < 0 || slot >= rg.S ? 0 : slot]);
+            return;
+        }
+    }
     const int s4 = s & ~A;
     const int lim = (int)(P.nnz & ~(long long)A);     // last entry reachable by bulk copies
     int e4 = (e + A) & ~A;
@@ -239,7 +259,7 @@ __device__ __forceinline__ RingPos ring_next_pass(const Ring& rg, RingPos p, int
 // by at most P.lookahead tiles until the consumers start that pass (ctl[3] counts the
 // passes they have started).  Its waits end through the stop flag (ctl[0], raised by the
 // consumers at the end of a persistent solve) or the CTA's watchdog flag (ctl[4]).
-template <bool CMP>
+template <bool CMP, bool CHK = false>
 __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, long long tb, int Tc,
                                               long long passes, int q, int NP) {
     const int lane = threadIdx.x & 31;
@@ -272,7 +292,7 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
             const int si = __shfl_sync(0xffffffffu, cached ? s : ps, cached ? j : l);
             const int ei = __shfl_sync(0xffffffffu, cached ? e : pe, cached ? j : l);
             ++issued;
-            if (lane == 0) producer_issue<CMP>(P, rg, j, tb + j, si, ei, policy, (unsigned)j + 1u, issued == fault_at);
+            if (lane == 0) producer_issue<CMP, CHK>(P, rg, j, tb + j, si, ei, policy, (unsigned)j + 1u, issued == fault_at);
         }
     }
     if (Ts <= 0 || Q <= 0) return;
@@ -316,8 +336,8 @@ __device__ __forceinline__ void producer_loop(const Params& P, const Ring& rg, l
             const int si = __shfl_sync(0xffffffffu, s, src);
             const int ei = __shfl_sync(0xffffffffu, e, src);
             ++issued;
-            if (lane == 0) producer_issue<CMP>(P, rg, Pn + (int)slot, tb + Pn + j, si, ei, policy, (unsigned)seq + 1u,
-                                               issued == fault_at);
+            if (lane == 0) producer_issue<CMP, CHK>(P, rg, Pn + (int)slot, tb + Pn + j, si, ei, policy, (unsigned)seq + 1u,
+                                                    issued == fault_at);
             seq += (unsigned long long)NP;
             j += NP;
             while (j >= Ts) { j -= Ts; ++pass; }
@@ -381,7 +401,7 @@ __device__ __forceinline__ double2 ld_global_f64x2(const double2* p) {
 // needs it from the pair {p_old[c], r[c]} (one 16-byte gather; K2 stored r there).  Same
 // operation, same operands, same bits as the owner's own update; it saves the third grid
 // synchronisation of an iteration.  `x` then points at the double2 pairs.
-template <int U, bool FOLD, bool CMP, bool GF>
+template <int U, bool FOLD, bool CMP, bool GF, bool CHK = false>
 __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, RingPos pos, int j,
                                                int lane, int row, double beta = 0.0) {
     static_assert(U % 3 == 0, "three accumulators");
@@ -420,6 +440,13 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
         ks = rp[lane] - base; ke = rp[lane + 1] - base;
         sc = rg.cols(slot);
     }
+    if constexpr (CHK) {
+        // row bounds inside the slot's value area (the streamlined trip also reads up to U values past a
+        // short row's end, unpredicated: those must still lie inside the slot)
+        const int shift = CMP ? (int)(sv - rg.vals(slot)) : 0;
+        const int room = (rg.slot_bytes / 8) - shift;
+        if (ks < 0 || ke < ks || ke + shift > rg.cap || ks + U > room) { chk_fail(rg); ks = 0; ke = 0; }
+    }
     const int trips = __reduce_max_sync(0xffffffffu, (ke - ks + U - 1) / U);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
     if constexpr (CMP && GF && !FOLD) {
@@ -436,8 +463,11 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
             double xv[U];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const unsigned code = __byte_perm(cw[u >> 2], 0u, 0x4440u | (unsigned)(u & 3));
-                xv[u] = ld_global_f64(x + (row + rg.offtab[code]));
+                unsigned code = __byte_perm(cw[u >> 2], 0u, 0x4440u | (unsigned)(u & 3));
+                if constexpr (CHK) { if ((int)code >= rg.ncodes) { chk_fail(rg); code = 0; } }
+                int col = row + rg.offtab[code];
+                if constexpr (CHK) { if (col < 0 || col >= rg.n) { chk_fail(rg); col = 0; } }
+                xv[u] = ld_global_f64(x + col);
             }
             const double* sr = sv + ks;
             const int len = ke - ks;
@@ -481,11 +511,13 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
             const int kk = in ? k + u : 0;
             int cc;
             if constexpr (CMP) {
-                const unsigned code = __byte_perm(cw[u >> 2], cw[(u >> 2) + 1 < NW ? (u >> 2) + 1 : NW - 1], cbase + (u & 3)) & 0xffu;
+                unsigned code = __byte_perm(cw[u >> 2], cw[(u >> 2) + 1 < NW ? (u >> 2) + 1 : NW - 1], cbase + (u & 3)) & 0xffu;
+                if constexpr (CHK) { if (in && (int)code >= rg.ncodes) { chk_fail(rg); code = 0; } }
                 cc = row + rg.offtab[in ? code : 0];
             } else {
                 cc = sc[kk];
             }
+            if constexpr (CHK) { if (in && (cc < 0 || cc >= rg.n)) { chk_fail(rg); cc = 0; } }
             c[u] = in ? cc : 0;
             if constexpr (!GF) { const double vv = sv[kk]; v[u] = in ? vv : 0.0; }
         }
@@ -534,7 +566,7 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
 
 // Shapes without producer warps (NP = 0; only when every tile is pinned): consumer warp w copies
 // its own tiles w, w + W, ... into their slots, once per kernel.
-template <int W, bool CMP>
+template <int W, bool CMP, bool CHK = false>
 __device__ __forceinline__ void consumers_pin_tiles(const Params& P, const Ring& rg, long long tb, int Tc) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (lane != 0) return;
@@ -543,8 +575,8 @@ __device__ __forceinline__ void consumers_pin_tiles(const Params& P, const Ring&
     for (int j = warp; j < Pn; j += W) {
         const int s = ld_stream_s32(P.rp_pad + (tb + j) * kTileRows);
         const int e = ld_stream_s32(P.rp_pad + (tb + j) * kTileRows + kTileRows);
-        producer_issue<CMP>(P, rg, j, tb + j, s, e, policy, (unsigned)j + 1u,
-                            P.inject_fault > 0 && blockIdx.x == 0 && j == P.inject_fault - 1);
+        producer_issue<CMP, CHK>(P, rg, j, tb + j, s, e, policy, (unsigned)j + 1u,
+                                 P.inject_fault > 0 && blockIdx.x == 0 && j == P.inject_fault - 1);
     }
 }
 
@@ -875,7 +907,7 @@ __device__ __forceinline__ void phase_zero_x_tiles(const Params& P, long long tb
 
 // K1 with vectors in global memory: y = A x over this CTA's tiles, for the pass that starts at
 // ring position `pos`; returns this thread's partial of x.y when DOT.
-template <int W, int U, bool DOT, bool CMP, bool GF>
+template <int W, int U, bool DOT, bool CMP, bool GF, bool CHK = false>
 __device__ __forceinline__ double phase_spmv_tiles(const Params& P, const Ring& rg, const double* x,
                                                    double* y, long long tb, int Tc, RingPos pos) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -884,7 +916,7 @@ __device__ __forceinline__ double phase_spmv_tiles(const Params& P, const Ring& 
         const long long row = (tb + j) * kTileRows + lane;
         double xr = 0.0;
         if (DOT && row < P.n) xr = ld_global_f64(x + row);      // early: off the critical path
-        const double acc = consume_tile<U, false, CMP, GF>(rg, x, pos, j, lane, (int)row);
+        const double acc = consume_tile<U, false, CMP, GF, CHK>(rg, x, pos, j, lane, (int)row);
         if (row < P.n) {
             y[row] = acc;
             if (DOT) dot = fma(acc, xr, dot);

@@ -29,13 +29,13 @@ __device__ __forceinline__ void decide_start(const Params& P, double rr, double 
     (void)warp
 
 // ---- cg_spmv: y = A x
-template <int W, int NP, int U, bool GF, bool CMP>
+template <int W, int NP, int U, bool GF, bool CMP, bool CHK = false>
 __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_spmv(Params P, const double* x, double* y) {
     CGS_PROLOGUE(W);
     ring_init(P, rg);
-    if (warp >= W) { producer_loop<CMP>(P, rg, tb, Tc, 1, warp - W, NP); return; }
-    if constexpr (NP == 0) consumers_pin_tiles<W, CMP>(P, rg, tb, Tc);
-    phase_spmv_tiles<W, U, false, CMP, GF>(P, rg, x, y, tb, Tc, RingPos{0u, 0u, 0u});
+    if (warp >= W) { producer_loop<CMP, CHK>(P, rg, tb, Tc, 1, warp - W, NP); return; }
+    if constexpr (NP == 0) consumers_pin_tiles<W, CMP, CHK>(P, rg, tb, Tc);
+    phase_spmv_tiles<W, U, false, CMP, GF, CHK>(P, rg, x, y, tb, Tc, RingPos{0u, 0u, 0u});
 }
 
 // ---- stand-alone kernels of loop modes 1 (graph) and 2 (stepwise).  They read Params from

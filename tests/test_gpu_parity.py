@@ -613,6 +613,71 @@ def test_single_reduction_cg_breakdown(bound, cgmod, algo):
     neg.close()
 
 
+# ---------------------------------------------------------------- the library's own memcheck
+
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_checked_spmv_clean_on_valid_matrices(bound, cfg):
+    """Option "checked": the SpMV with every index validated on the device (bulk-copy source ranges,
+    slot offsets, index codes, gathered columns).  On valid matrices it must count nothing, in every
+    kernel shape and slot format, pinned and streamed, and return the unchecked kernel's bits."""
+    B = bound(cfg)
+    xv = dev(gi.seeded_vector(400 + cfg, B.p.n))
+    for spmv in (2, 3, 4):
+        for compress in (1, 0):
+            for pin in (1, 0):
+                for k, v in (("spmv", spmv), ("compress", compress), ("pin", pin)):
+                    B.cg.set_option(k, v)
+                if B.cg.info("spmv") != spmv:
+                    continue
+                y0 = B.cg.spmv(xv)
+                B.cg.set_option("checked", 1)
+                y1 = B.cg.spmv(xv)
+                B.cg.set_option("checked", 0)
+                assert B.cg.info("check_errors") == 0 and torch.equal(y0, y1), (spmv, compress, pin)
+    for k, v in (("spmv", 0), ("compress", 1), ("pin", 1)):
+        B.cg.set_option(k, v)
+
+
+@pytest.mark.parametrize("n,max_len,empty_every", [(33, 40, 0), (1000, 31, 7), (4097, 70, 5)])
+def test_checked_spmv_clean_on_ragged_matrices(cgmod, n, max_len, empty_every):
+    rp, ci, va = _random_csr(n, 1000 + n, max_len, empty_every, unsorted=True)
+    A = cgmod.CG(dev(rp), dev(ci), dev(va))
+    xv = dev(gi.seeded_vector(5, n))
+    for spmv in (2, 3, 4):
+        A.set_option("spmv", spmv)
+        if A.info("spmv") != spmv:
+            continue
+        y0 = A.spmv(xv)
+        A.set_option("checked", 1)
+        y1 = A.spmv(xv)
+        A.set_option("checked", 0)
+        assert A.info("check_errors") == 0 and torch.equal(y0, y1)
+    A.close()
+
+
+@pytest.mark.parametrize("compress", [False, True])
+@pytest.mark.parametrize("bad_col", [-3, 5])
+def test_checked_spmv_catches_a_corrupt_column(cgmod, problems, compress, bad_col):
+    """A column index outside [0, n) (relative to n for the positive case): the checked SpMV counts
+    it, never dereferences it, reports CG_ECUDA, and leaves the device usable."""
+    p = problems(0)
+    ci = p.colind.copy()
+    ci[1234] = bad_col if bad_col < 0 else p.n + bad_col
+    A = cgmod.CG(dev(p.rowptr), dev(ci), dev(p.vals), compress=compress)
+    assert not A.check_csr()
+    A.set_option("checked", 1)
+    xv = dev(gi.seeded_vector(1, p.n))
+    with pytest.raises(cgmod.CGError) as err:
+        A.spmv(xv)
+    assert err.value.code == -2 and "caught" in str(err.value) and A.info("check_errors") >= 1
+    A.close()
+    good = cgmod.CG(dev(p.rowptr), dev(p.colind), dev(p.vals))
+    good.set_option("checked", 1)
+    good.spmv(xv)
+    assert good.info("check_errors") == 0
+    good.close()
+
+
 # ---------------------------------------------------------------- watchdog
 
 @pytest.mark.parametrize("compress,loop,spmv", [(1, 0, 0), (0, 0, 0), (0, 2, 3), (1, 1, 2)])
