@@ -3,6 +3,7 @@
 #include "../../include/cg.h"
 #include "cg_kernels.cuh"
 #include "cg_stream_kernels.cuh"
+#include "cg_variants.h"
 
 #include <math.h>
 #include <stdlib.h>
@@ -431,59 +432,19 @@ static thread_local char g_cuda_err[256] = "no CUDA error recorded";
         }                                                                     \
     } while (0)
 
-// Streamed variants: W consumer warps, NP producer warps, U entries in flight per lane
-// (cg_stream.cuh).  "spmv" option value = index + 2.  Every kernel that touches the ring exists
-// for both slot formats ([cmp]: 0 plain CSR, 1 compressed index).
-enum PersistentKind { kR0, kR0Jacobi, kR2, kR2Jacobi, kR2Fold, kR4, kR4Jacobi, kR4Fold, kNumPersistent };
-struct StreamFns {
-    int W, NP, U;
-    const void* spmv[2];
-    const void* spmv_checked[2];           // option "checked"
-    const void* init_spmv[2]; const void* init_residual; const void* init_scalars;
-    const void* k1[2]; const void* k2; const void* k3;
-    const void* persistent[2][kNumPersistent];
-    const void* cg1[2][2];                 // option "algo" = 1 (Chronopoulos-Gear): [cmp][R == 4]
-    const void* pipe[2][2];                // option "algo" = 2 (pipelined CG)
-};
-
-template <int W, int NP, int U, bool GF, bool CMP> static void fill_cmp_fns(StreamFns& f) {
-    constexpr int c = CMP ? 1 : 0;
-    f.spmv[c] = (const void*)cgs::ks_spmv<W, NP, U, GF, CMP>;
-    f.spmv_checked[c] = (const void*)cgs::ks_spmv<W, NP, U, GF, CMP, true>;
-    f.init_spmv[c] = (const void*)cgs::ks_init_spmv<W, NP, U, GF, CMP>;
-    f.k1[c] = (const void*)cgs::ks1_spmv_dot<W, NP, U, GF, CMP>;
-    f.persistent[c][kR0]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 0, false, false, CMP>;
-    f.persistent[c][kR0Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 0, true, false, CMP>;
-    f.persistent[c][kR2]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 2, false, false, CMP>;
-    f.persistent[c][kR2Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 2, true, false, CMP>;
-    f.persistent[c][kR2Fold]   = (const void*)cgs::ks_persistent<W, NP, U, GF, 2, false, true, CMP>;
-    f.persistent[c][kR4]       = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, false, CMP>;
-    f.persistent[c][kR4Jacobi] = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, true, false, CMP>;
-    f.persistent[c][kR4Fold]   = (const void*)cgs::ks_persistent<W, NP, U, GF, 4, false, true, CMP>;
-    f.cg1[c][0] = (const void*)cgs::ks_persistent_cg1<W, NP, U, GF, 2, CMP>;
-    f.cg1[c][1] = (const void*)cgs::ks_persistent_cg1<W, NP, U, GF, 4, CMP>;
-    if constexpr (NP != 4) {               // the single- and no-reduction loops exist for shapes 3 and 4 only (build time)
-        f.pipe[c][0] = (const void*)cgs::ks_persistent_pipe<W, NP, U, GF, 2, CMP>;
-        f.pipe[c][1] = (const void*)cgs::ks_persistent_pipe<W, NP, U, GF, 4, CMP>;
-    } else {
-        f.pipe[c][0] = f.pipe[c][1] = nullptr;
-    }
-}
-template <int W, int NP, int U, bool GF> static StreamFns make_stream_fns() {
-    StreamFns f;
-    f.W = W; f.NP = NP; f.U = U;
-    f.init_residual = (const void*)cgs::ks_init_residual<W, NP>;
-    f.init_scalars = (const void*)cgs::ks_init_scalars<W, NP>;
-    f.k2 = (const void*)cgs::ks2_update_xr<W, NP>;
-    f.k3 = (const void*)cgs::ks3_update_p<W, NP>;
-    fill_cmp_fns<W, NP, U, GF, false>(f);
-    fill_cmp_fns<W, NP, U, GF, true>(f);
-    return f;
-}
-static constexpr int kNumStream = 3;
+// Streamed kernel shapes: their kernels are instantiated in cg_variant.cu, one translation unit per
+// (shape, slot format) so that the build can compile them in parallel (cg_variants.h).
+static constexpr int kNumStream = kNumShapes;
 static const StreamFns& stream_fns(int idx) {
-    static const StreamFns table[kNumStream] = {make_stream_fns<12, 4, 9, false>(), make_stream_fns<11, 5, 9, false>(),
-                                                make_stream_fns<16, 0, 27, true>()};
+    static StreamFns table[kNumStream];
+    static bool ready = false;
+    if (!ready) {
+        memset(table, 0, sizeof(table));
+        cg_fill_fns_0_0(table[0]); cg_fill_fns_0_1(table[0]);
+        cg_fill_fns_1_0(table[1]); cg_fill_fns_1_1(table[1]);
+        cg_fill_fns_2_0(table[2]); cg_fill_fns_2_1(table[2]);
+        ready = true;
+    }
     return table[idx];
 }
 
