@@ -618,7 +618,7 @@ def main():
     # rtol = 0, maxit = K (2000 for configs 0-3, 200 for config 4): throughput that does not depend on
     # where convergence falls; plus the SpMV alone (cg_spmv), the to-convergence solve of configs 0-3,
     # and the oracle on the same fixed work (K = 200 / 20) on one host core.
-    if rank == 0 and not args.no_per_config:
+    if rank == 0 and world == 1 and not args.no_per_config:
         per = {}
         for cfg in (0, 1, 2, 3, 4):
             if cfg == 4 and args.no_160:
