@@ -338,3 +338,29 @@ def test_openmp_baseline_matches_the_oracle(problems):
         assert abs(got.iters - ref.iters) <= max(1, int(0.02 * ref.iters))
         assert np.linalg.norm(got.x - ref.x) / np.linalg.norm(ref.x) <= 1e-8
         assert got.status == ref.status == 0
+
+
+def test_stored_config4_run_matches_the_live_oracle():
+    """tests/golden/config4_converged.npz (the oracle's 41-minute solve of the 160^3 config) cannot be
+    recomputed in a test; its 48^3 sibling, written by the same committed script in the same way, can:
+    the live oracle must reproduce it bit for bit, and both files must carry the generator's hash."""
+    import hashlib
+    import os
+    import cg_inputs as gi
+    from oracle import cg_oracle as orc
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    small = np.load(os.path.join(gdir, "config4_grid48_converged.npz"))
+    p = gi.make_config(4, grid=48)
+    h = hashlib.sha256()
+    for a in (p.rowptr, p.colind, p.vals, p.b):
+        h.update(np.ascontiguousarray(a).view(np.uint8).data)
+    assert h.hexdigest() == str(small["generator_sha256"])
+    ref = orc.cg(p.rowptr, p.colind, p.vals, p.b, rtol=p.rtol, maxit=p.maxit)
+    assert ref.iters == int(small["iters"]) and ref.status == int(small["status"]) == 0
+    assert np.array_equal(ref.hist, small["hist"])
+    rows = small["x_rows"]
+    assert np.array_equal(ref.x[rows], small["x_sample"])
+    big = np.load(os.path.join(gdir, "config4_converged.npz"))
+    assert int(big["n"]) == 160 ** 3 and int(big["status"]) == 0 and len(big["hist"]) == int(big["iters"]) + 1
+    assert float(big["true_relres"]) <= 2e-8 and big["hist"][-1] <= 1e-8 * float(big["bnorm"])
+    assert np.all(np.isfinite(big["hist"])) and len(str(big["generator_sha256"])) == 64
