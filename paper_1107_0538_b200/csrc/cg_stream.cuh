@@ -382,6 +382,41 @@ __device__ __forceinline__ double2 ld_global_f64x2(const double2* p) {
     return v;
 }
 
+// The trip of a tile whose rows all have <= UU entries, compressed index, gather-first: UU gathers are
+// issued back to back, the values are read from the slot while they fly, then the DFMAs run in CSR order
+// into three accumulators.  The record pads short rows with the code of offset 0, so every padding
+// gather reads x[row] (a valid address) and only the DFMA is predicated: ~10 instead of ~22
+// instructions per entry -- the pinned kernel is bound by instruction issue and by the shared-memory
+// datapath (ncu: 21 k warp instructions per SM and iteration through 4 schedulers in ~8 k cycles).
+// sw: this lane's code words (word g at sw[32 g]); sr: the row's first value; len: its length.
+template <int UU, bool CHK>
+__device__ __forceinline__ double streamlined_trip(const Ring& rg, const double* x, const unsigned* sw, int gmax,
+                                                   const double* sr, int len, int row) {
+    static_assert(UU % 3 == 0, "three accumulators");
+    constexpr int NW = (UU + 3) / 4;
+    unsigned cw[NW];
+#pragma unroll
+    for (int g = 0; g < NW; ++g) cw[g] = sw[32 * (g < gmax ? g : gmax)];
+    double xv[UU];
+#pragma unroll
+    for (int u = 0; u < UU; ++u) {
+        unsigned code = __byte_perm(cw[u >> 2], 0u, 0x4440u | (unsigned)(u & 3));
+        if constexpr (CHK) { if ((int)code >= rg.ncodes) { chk_fail(rg); code = 0; } }
+        int col = row + rg.offtab[code];
+        if constexpr (CHK) { if (col < 0 || col >= rg.n) { chk_fail(rg); col = 0; } }
+        xv[u] = ld_global_f64(x + col);
+    }
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+#pragma unroll
+    for (int u = 0; u < UU; u += 3) {
+        const double v0 = sr[u], v1 = sr[u + 1], v2 = sr[u + 2];
+        if (u < len)     a0 = fma(v0, xv[u], a0);
+        if (u + 1 < len) a1 = fma(v1, xv[u + 1], a1);
+        if (u + 2 < len) a2 = fma(v2, xv[u + 2], a2);
+    }
+    return (a0 + a1) + a2;
+}
+
 // One tile: wait for its slot, y_row = sum_k a_k x[col_k] for this lane's row.  U entries are
 // in flight per lane and trip: their column indices and values are read from shared memory,
 // then the U gathers are issued, then the FMAs go into three independent accumulators
@@ -447,42 +482,24 @@ __device__ __forceinline__ double consume_tile(const Ring& rg, const double* x, 
         const int room = (rg.slot_bytes / 8) - shift;
         if (ks < 0 || ke < ks || ke + shift > rg.cap || ks + U > room) { chk_fail(rg); ks = 0; ke = 0; }
     }
-    const int trips = __reduce_max_sync(0xffffffffu, (ke - ks + U - 1) / U);
+    const int tmax = __reduce_max_sync(0xffffffffu, ke - ks);      // longest row of the tile (warp-uniform)
+    const int trips = (tmax + U - 1) / U;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
     if constexpr (CMP && GF && !FOLD) {
         // Streamlined trip for the common case: every row of the tile fits one trip and the tile is not
-        // the ragged last one.  The record pads short rows with the code of offset 0, so every
-        // padding gather reads x[row] (a valid address) and only the DFMA is predicated: ~10 instead
-        // of ~22 instructions per entry -- the pinned kernel is bound by instruction issue
-        // (ncu: 21 k warp instructions per SM and iteration through 4 schedulers in ~8 k cycles).
+        // the ragged last one (streamlined_trip below).  Its length follows the tile's longest row in steps
+        // of 9 entries: a tile of 7-point rows issues 9 gathers, not 27, and the 18-entry rows of a boundary
+        // plane (whose values sit 18 doubles apart: two-way bank conflicts) read 18 values, not 27.
         if (trips == 1 && row - lane + (kTileRows - 1) < rg.n) {
-            constexpr int NW = (U + 3) / 4;
-            unsigned cw[NW];
-#pragma unroll
-            for (int g = 0; g < NW; ++g) cw[g] = sw[32 * (g < gmax ? g : gmax)];
-            double xv[U];
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                unsigned code = __byte_perm(cw[u >> 2], 0u, 0x4440u | (unsigned)(u & 3));
-                if constexpr (CHK) { if ((int)code >= rg.ncodes) { chk_fail(rg); code = 0; } }
-                int col = row + rg.offtab[code];
-                if constexpr (CHK) { if (col < 0 || col >= rg.n) { chk_fail(rg); col = 0; } }
-                xv[u] = ld_global_f64(x + col);
-            }
-            const double* sr = sv + ks;
-            const int len = ke - ks;
-#pragma unroll
-            for (int u = 0; u < U; u += 3) {
-                const double v0 = sr[u], v1 = sr[u + 1], v2 = sr[u + 2];
-                if (u < len)     a0 = fma(v0, xv[u], a0);
-                if (u + 1 < len) a1 = fma(v1, xv[u + 1], a1);
-                if (u + 2 < len) a2 = fma(v2, xv[u + 2], a2);
-            }
+            double acc;
+            if (U > 18 && tmax > 18)     acc = streamlined_trip<(U > 18 ? U : 9), CHK>(rg, x, sw, gmax, sv + ks, ke - ks, row);
+            else if (U > 9 && tmax > 9)  acc = streamlined_trip<(U > 9 ? 18 : 9), CHK>(rg, x, sw, gmax, sv + ks, ke - ks, row);
+            else                         acc = streamlined_trip<9, CHK>(rg, x, sw, gmax, sv + ks, ke - ks, row);
             if (!pinned) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&rg.empty[slot]);
             }
-            return (a0 + a1) + a2;
+            return acc;
         }
     }
     if (trips == 0 && !pinned) {
