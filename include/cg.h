@@ -165,8 +165,13 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               1 = fold K3 into the next K1 (every gathered p_j is recomputed on the fly as
  *               fma(beta, p_old_j, r_j) from one 16-byte {p_old, r} pair, the owner's own
  *               expression, so results keep their bits) and synchronise the grid twice
- *               instead of three times per iteration; 0 = off; 2 (default) = on when a CTA has
- *               <= 8 tiles or its whole slice of the matrix is pinned in shared memory
+ *               instead of three times per iteration; 0 = off; 2 (default) = on when a CTA
+ *               gathers <= 500 entries per lane-row set (tiles x mean row length) and the
+ *               short-row kernels do not apply
+ *   "short_rows" 1 (default) = when no row has more than 9 entries (the 7-point Laplacian), every
+ *               CTA's slice is pinned and a consumer warp owns several tiles, run the kernels
+ *               that keep the gathers of 2-3 tiles in flight per warp instead of one tile's 9
+ *               (same operations per row in the same order: same bits); 0 = off
  *   "pin"       1 (default) = when every CTA's slice of the matrix fits the shared memory (up
  *               to 64 tiles per SM) and the matrix would otherwise be re-read from the L2 every
  *               iteration, copy it there once per solve and keep it; 0 = stream everything
@@ -208,7 +213,7 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
  * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "pinned_tiles", "slot_bytes",
- * "resident_rows", "fold", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
+ * "resident_rows", "fold", "short_rows", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
  * counted by the last checked cg_spmv), "lines_per_gather_x100"
  * (cg_create statistic: 128-byte lines one warp-wide gather touches on average, times 100).
  * Unknown names return CG_EINVAL. */

@@ -1,7 +1,7 @@
 """Build libcg_b200.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo).
 
-cg_api.cu (ABI, setup kernels, generic path) and six instances of cg_variant.cu (one per streamed
-kernel shape and slot format) are compiled in parallel and linked into one shared library."""
+cg_api.cu (ABI, setup kernels, generic path) and seven instances of cg_variant.cu (one per streamed
+kernel shape and slot format, one for the short-row kernels) are compiled in parallel and linked into one shared library."""
 from __future__ import annotations
 
 import os
@@ -41,6 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with tempfile.TemporaryDirectory(prefix="cg_b200_build_") as tmp:
         units = [("api", SOURCES[0], [])]
         units += [(f"shape{s}_cmp{c}", SOURCES[1], [f"-DCG_SHAPE={s}", f"-DCG_CMP={c}"]) for s in range(3) for c in range(2)]
+        units += [("short", SOURCES[1], ["-DCG_SHORT"])]
         procs = []
         for name, src, defs in units:
             obj = os.path.join(tmp, name + ".o")

@@ -443,6 +443,7 @@ static const StreamFns& stream_fns(int idx) {
         cg_fill_fns_0_0(table[0]); cg_fill_fns_0_1(table[0]);
         cg_fill_fns_1_0(table[1]); cg_fill_fns_1_1(table[1]);
         cg_fill_fns_2_0(table[2]); cg_fill_fns_2_1(table[2]);
+        cg_fill_fns_short(table[2]);
         ready = true;
     }
     return table[idx];
@@ -471,7 +472,7 @@ struct cg_handle {
     int sms, smem_optin, clock_khz;
     size_t l2_bytes;
     int loop, spmv_opt, chunk, ctas_per_sm, resident_opt, lookahead, max_slots, fold_opt, pin_opt, compress_opt;
-    int spin_budget_ms, inject_fault, algo_opt, checked_opt;
+    int spin_budget_ms, inject_fault, algo_opt, checked_opt, short_opt;
     int max_row_len, max_tile_nnz, tpr;
     double lines_per_gather;               // cg_create statistic (k_gather_stats)
     int smem_cap_kb;                       // option: 0 = auto
@@ -482,7 +483,7 @@ struct cg_handle {
     cudaStream_t cap_stream;               // capture-only stream (the legacy stream cannot capture)
     unsigned long long* trace; int trace_iters;
     long long launches;
-    int last_resident, last_fold;          // what the last persistent solve used (info)
+    int last_resident, last_fold, last_short;      // what the last persistent solve used (info)
     int last_chk_errors;                   // violations counted by the last checked cg_spmv
 };
 
@@ -623,11 +624,23 @@ static int resident_rows(const cg_handle* h, int v) {
     return need <= 2 ? 2 : need <= 4 ? 4 : 0;        // 8 rows per thread spill and gain nothing (measured on config 1)
 }
 
+// Short-row kernels (option "short_rows": 0 off, 1 auto): shape 2 with the compressed index, every tile pinned,
+// no row longer than 9 entries (the 7-point Laplacian), more than one tile per consumer warp, vectors in
+// registers.  They keep several tiles' gathers in flight per warp (cg_stream.cuh: short_batch).
+static bool short_rows_possible(const cg_handle* h, int v, const Geo& g) {
+    if (!h->short_opt || v != 4 || !g.cmp || resident_rows(h, v) == 0) return false;
+    if (stream_fns(2).short_persistent[0] == nullptr) return false;
+    const int W = stream_fns(2).W;
+    return h->max_row_len <= 9 && g.pinned >= tiles_per_cta_max(h) && tiles_per_cta_max(h) > W;
+}
+
 // Folding K3 into the next K1 trades a grid synchronisation for a 16-byte gather per entry
 // instead of an 8-byte one.  Option "fold": 0 off, 1 on, 2 auto.
 static bool fold_effective(const cg_handle* h, int v, int precond, const Geo& g) {
     if (precond || resident_rows(h, v) == 0) return false;
     if (h->fold_opt != 2) return h->fold_opt == 1;
+    // auto: where the short-row kernels apply they win (config 1: 8.9 against 10.6 us per iteration folded)
+    if (short_rows_possible(h, v, g)) return false;
     // auto: the 16-byte gathers must cost less than the synchronisation they save.  Measured
     // (us per iteration, folded / not): config 0 (1 tile of 24 entries per row per CTA) 7.4 / 7.8,
     // config 1 (56 pinned tiles x 7) 10.6 / 13.4, config 2 (29 pinned tiles x 26) 10.8 / 10.4.
@@ -713,7 +726,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     h->clock_khz = khz > 0 ? khz : 2000000;
     h->l2_bytes = (size_t)prop.l2CacheSize;
     h->loop = 0; h->spmv_opt = 0; h->chunk = 32; h->ctas_per_sm = 0; h->resident_opt = 1;
-    h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->pin_opt = 1; h->compress_opt = 1;
+    h->lookahead = 1 << 30; h->max_slots = cgs::kMaxSlots; h->fold_opt = 2; h->pin_opt = 1; h->compress_opt = 1; h->short_opt = 1;
     h->spin_budget_ms = 2000; h->inject_fault = 0;
 
     cudaError_t e = cudaHostAlloc((void**)&h->h_scal, sizeof(Scal), cudaHostAllocDefault);
@@ -764,6 +777,9 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
                 if (f.pipe[c][k]) CKH(cudaFuncSetAttribute(f.pipe[c][k], cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
             }
         }
+        const void* shorts[] = {f.short_persistent[0], f.short_persistent[1], f.short_cg1, f.short_pipe};
+        for (const void* fn : shorts)
+            if (fn) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
     }
     *out = h;
     return CG_OK;
@@ -869,6 +885,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!strcmp(name, "smem_cap_kb")) { if (value < 0 || value > 227) return CG_EINVAL; h->smem_cap_kb = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
+    if (!strcmp(name, "short_rows")) { if (value < 0 || value > 1) return CG_EINVAL; h->short_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "spin_budget_ms")) { if (value < 1 || value > 600000) return CG_EINVAL; h->spin_budget_ms = (int)value; return CG_OK; }
     if (!strcmp(name, "inject_fault")) { if (value < 0 || value > (1 << 30)) return CG_EINVAL; h->inject_fault = (int)value; return CG_OK; }
@@ -909,6 +926,7 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "resident_rows")) *value = resident_rows(h, v);
     else if (!strcmp(name, "fold")) *value = fold_effective(h, v, 0, g) ? 1 : 0;
     else if (!strcmp(name, "algo")) *value = algo_effective(h, v, 0);
+    else if (!strcmp(name, "short_rows")) *value = (short_rows_possible(h, v, g) && !(fold_effective(h, v, 0, g) && algo_effective(h, v, 0) == 0)) ? 1 : 0;
     else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
     else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
     else if (!strcmp(name, "from_hbm")) *value = g.from_hbm ? 1 : 0;
@@ -1122,6 +1140,12 @@ static int solve_impl(cg_handle* h, const double* d_b, double* d_x, double rtol,
             const int algo = algo_effective(h, v, precond);
             const void* fn = algo == 1 ? f.cg1[g.cmp][R == 4 ? 1 : 0] : algo == 2 ? f.pipe[g.cmp][R == 4 ? 1 : 0]
                                        : f.persistent[g.cmp][kind];
+            // short rows, every tile pinned, vectors in registers: the kernels that keep several tiles' gathers in flight
+            h->last_short = 0;
+            if (short_rows_possible(h, v, g) && !(fold && algo == 0)) {
+                fn = algo == 1 ? f.short_cg1 : algo == 2 ? f.short_pipe : f.short_persistent[precond ? 1 : 0];
+                h->last_short = 1; h->last_resident = 4;
+            }
             CK(cudaMemsetAsync(h->bslots, 0xFF, kBslotBytes, st));        // arm the all-reduce slots
             CK(cudaLaunchCooperativeKernel(fn, dim3(G), dim3(32 * (f.W + f.NP)), args, g.smem, st));
         }

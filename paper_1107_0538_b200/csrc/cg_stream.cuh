@@ -390,14 +390,12 @@ __device__ __forceinline__ double2 ld_global_f64x2(const double2* p) {
 // datapath (ncu: 21 k warp instructions per SM and iteration through 4 schedulers in ~8 k cycles).
 // sw: this lane's code words (word g at sw[32 g]); sr: the row's first value; len: its length.
 template <int UU, bool CHK>
-__device__ __forceinline__ double streamlined_trip(const Ring& rg, const double* x, const unsigned* sw, int gmax,
-                                                   const double* sr, int len, int row) {
-    static_assert(UU % 3 == 0, "three accumulators");
+__device__ __forceinline__ void trip_issue(const Ring& rg, const double* x, const unsigned* sw, int gmax, int row,
+                                           double (&xv)[UU]) {
     constexpr int NW = (UU + 3) / 4;
     unsigned cw[NW];
 #pragma unroll
     for (int g = 0; g < NW; ++g) cw[g] = sw[32 * (g < gmax ? g : gmax)];
-    double xv[UU];
 #pragma unroll
     for (int u = 0; u < UU; ++u) {
         unsigned code = __byte_perm(cw[u >> 2], 0u, 0x4440u | (unsigned)(u & 3));
@@ -406,6 +404,10 @@ __device__ __forceinline__ double streamlined_trip(const Ring& rg, const double*
         if constexpr (CHK) { if (col < 0 || col >= rg.n) { chk_fail(rg); col = 0; } }
         xv[u] = ld_global_f64(x + col);
     }
+}
+template <int UU>
+__device__ __forceinline__ double trip_finish(const double* sr, int len, const double (&xv)[UU]) {
+    static_assert(UU % 3 == 0, "three accumulators");
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
 #pragma unroll
     for (int u = 0; u < UU; u += 3) {
@@ -415,6 +417,58 @@ __device__ __forceinline__ double streamlined_trip(const Ring& rg, const double*
         if (u + 2 < len) a2 = fma(v2, xv[u + 2], a2);
     }
     return (a0 + a1) + a2;
+}
+template <int UU, bool CHK>
+__device__ __forceinline__ double streamlined_trip(const Ring& rg, const double* x, const unsigned* sw, int gmax,
+                                                   const double* sr, int len, int row) {
+    double xv[UU];
+    trip_issue<UU, CHK>(rg, x, sw, gmax, row, xv);
+    return trip_finish<UU>(sr, len, xv);
+}
+
+// Short rows (every row of the tile has <= 9 entries: the 7-point Laplacian), tiles pinned: one tile's trip
+// keeps only 9 gathers in flight and a warp that owns several tiles would pay one exposed L2 round trip per
+// tile.  short_batch issues the gathers of NB <= 3 tiles (27 in flight, as a 27-point tile has) before it
+// finishes any of them.  Per row the operations and their order are those of streamlined_trip<9>: same bits.
+// Only for tiles that have landed and were checked by tiles_are_short (their "full" barrier is not waited
+// on again: a pinned slot has one phase for the whole launch).
+template <int NB, int W>
+__device__ __forceinline__ void short_batch(const Ring& rg, const double* x, int warp, int kk0, int lane,
+                                            long long tb, double* out) {
+    // no branch in here: a gather result that is defined on one path only is merged through local memory,
+    // and the store that does it waits for the gather (measured: the batch then runs slower than tile by tile)
+    double xv[NB][9];
+    const int row0 = (int)(tb * kTileRows) + lane;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const int j = warp + (kk0 + b) * W;
+        trip_issue<9, false>(rg, x, reinterpret_cast<const unsigned*>(rg.rec(j) + kRecHdr) + lane, rg.rec_words - 1,
+                             row0 + j * kTileRows, xv[b]);
+    }
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const int j = warp + (kk0 + b) * W;
+        const unsigned short* hd = reinterpret_cast<const unsigned short*>(rg.rec(j));
+        const int ks = hd[lane], ke = hd[lane + 1];
+        out[kk0 + b] = trip_finish<9>(rg.vals(j) + hd[33] + ks, ke - ks, xv[b]);
+    }
+}
+
+// True (in every lane) when all tiles of this warp are pinned, complete (not the ragged last tile) and have
+// only rows of <= 9 entries.  Call after a pass over the tiles (the slots' contents must have landed).
+template <int W, int R>
+__device__ __forceinline__ bool tiles_are_short(const Ring& rg, int warp, int lane, long long tb, int Tc) {
+    bool ok = rg.P >= Tc;
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        if (ok && j < Tc) {
+            const unsigned short* hd = reinterpret_cast<const unsigned short*>(rg.rec(j));
+            const int tmax = __reduce_max_sync(0xffffffffu, (int)hd[lane + 1] - (int)hd[lane]);
+            ok = tmax <= 9 && (tb + j) * kTileRows + (kTileRows - 1) < rg.n;
+        }
+    }
+    return ok;
 }
 
 // One tile: wait for its slot, y_row = sum_k a_k x[col_k] for this lane's row.  U entries are
@@ -956,6 +1010,38 @@ __device__ __forceinline__ double phase_spmv_tiles(const Params& P, const Ring& 
         }
     }
     return dot;
+}
+
+// The kernels instantiated gather-first with U = 9 are the short-row kernels (cg_variant.cu, CG_SHORT).
+template <int U, bool GF, bool CMP, int R> struct ShortBatchKernel { static constexpr bool value = GF && CMP && U == 9 && R > 1; };
+
+// K1 of a consumer thread that keeps its rows in registers: out[kk] = (A x)_row of tile warp + kk W
+// (untouched when the warp has no such tile).  batch (warp-uniform, from tiles_are_short) selects short_batch.
+template <int W, int U, int R, bool CMP, bool GF>
+__device__ __forceinline__ void k1_resident_tiles(const Ring& rg, const double* x, RingPos pos, int warp, int lane,
+                                                  long long tb, int Tc, bool batch, double (&out)[R]) {
+    if constexpr (ShortBatchKernel<U, GF, CMP, R>::value) {
+        if (batch) {
+            // the warp's tiles are warp, warp + W, ...: cnt of them (warp-uniform); one branch-free batch per case
+            const int cnt = Tc > warp ? (Tc - warp + W - 1) / W : 0;
+            if (R >= 4 && cnt >= 4) {
+                short_batch<2, W>(rg, x, warp, 0, lane, tb, out);
+                short_batch<2, W>(rg, x, warp, 2, lane, tb, out);
+            } else if (R >= 3 && cnt == 3) {
+                short_batch<3, W>(rg, x, warp, 0, lane, tb, out);
+            } else if (cnt == 2) {
+                short_batch<2, W>(rg, x, warp, 0, lane, tb, out);
+            } else if (cnt == 1) {
+                short_batch<1, W>(rg, x, warp, 0, lane, tb, out);
+            }
+            return;
+        }
+    }
+#pragma unroll
+    for (int kk = 0; kk < R; ++kk) {
+        const int j = warp + kk * W;
+        if (j < Tc) out[kk] = consume_tile<U, false, CMP, GF>(rg, x, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+    }
 }
 
 }  // namespace cgs

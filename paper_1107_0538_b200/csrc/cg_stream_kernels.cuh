@@ -255,6 +255,11 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
         phase_init_tiles<W, PRE>(P, tb, Tc, arr, abb, arz);     // reads only this thread's own q
     }
     ++pass; pos = ring_next_pass(rg, pos, Tc);
+    // Short-row kernels (gather-first with U = 9: the host picks them when no row has more than 9 entries):
+    // a warp whose tiles are all pinned and complete keeps several tiles' gathers in flight (short_batch).
+    constexpr bool SB = ShortBatchKernel<U, GF, CMP, R>::value && !FOLD;
+    bool batch = false;
+    if constexpr (SB) batch = tiles_are_short<W, R>(rg, warp, lane, tb, Tc);
     double rr, bb, rz;
     bool dead;
     {
@@ -320,12 +325,19 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
                 }
                 cur ^= 1;
             } else {
+                if constexpr (SB) {
+                    k1_resident_tiles<W, U, R, CMP, GF>(rg, P.p, pos, warp, lane, tb, Tc, batch, qv);
 #pragma unroll
-                for (int kk = 0; kk < R; ++kk) {
-                    const int j = warp + kk * W;
-                    if (j < Tc) {
-                        qv[kk] = consume_tile<U, false, CMP, GF>(rg, P.p, pos, j, lane, (int)((tb + j) * kTileRows + lane));
-                        if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                    for (int kk = 0; kk < R; ++kk)
+                        if (warp + kk * W < Tc && row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                } else {
+#pragma unroll
+                    for (int kk = 0; kk < R; ++kk) {
+                        const int j = warp + kk * W;
+                        if (j < Tc) {
+                            qv[kk] = consume_tile<U, false, CMP, GF>(rg, P.p, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+                            if (row[kk] >= 0) dot = fma(qv[kk], pv[kk], dot);
+                        }
                     }
                 }
             }
@@ -480,6 +492,9 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
     bool dead = iter_sync<W, Plan, 0>(P, rg, bcount, nbar, cta, G, none);          // r0 is published
     double agam = 0.0, adel = 0.0;
     consumers_begin_pass(rg, pass);
+    constexpr bool SB = ShortBatchKernel<U, GF, CMP, R>::value;
+    bool batch = false;
+    if constexpr (SB) batch = tiles_are_short<W, R>(rg, warp, lane, tb, Tc);
 #pragma unroll
     for (int kk = 0; kk < R; ++kk) {
         const int j = warp + kk * W;
@@ -533,12 +548,19 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
         // K1: w = A r, partials of gamma' = r.r and delta = w.r
         agam = 0.0; adel = 0.0;
         consumers_begin_pass(rg, pass);
+        if constexpr (SB) {
+            k1_resident_tiles<W, U, R, CMP, GF>(rg, rpub, pos, warp, lane, tb, Tc, batch, wv);
 #pragma unroll
-        for (int kk = 0; kk < R; ++kk) {
-            const int j = warp + kk * W;
-            if (j < Tc) {
-                wv[kk] = consume_tile<U, false, CMP, GF>(rg, rpub, pos, j, lane, (int)((tb + j) * kTileRows + lane));
-                if (row[kk] >= 0) { agam = fma(rv[kk], rv[kk], agam); adel = fma(wv[kk], rv[kk], adel); }
+            for (int kk = 0; kk < R; ++kk)
+                if (warp + kk * W < Tc && row[kk] >= 0) { agam = fma(rv[kk], rv[kk], agam); adel = fma(wv[kk], rv[kk], adel); }
+        } else {
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) {
+                const int j = warp + kk * W;
+                if (j < Tc) {
+                    wv[kk] = consume_tile<U, false, CMP, GF>(rg, rpub, pos, j, lane, (int)((tb + j) * kTileRows + lane));
+                    if (row[kk] >= 0) { agam = fma(rv[kk], rv[kk], agam); adel = fma(wv[kk], rv[kk], adel); }
+                }
             }
         }
         ++pass; pos = ring_next_pass(rg, pos, Tc);
@@ -684,6 +706,9 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_pipe(
     bool dead = grid_barrier_partials<W>(P, rg, nbar, G, cta, 0, 0.0, 0.0, abb);            // r0 and b.b are published
     double agam = 0.0, adel = 0.0;
     consumers_begin_pass(rg, pass);
+    constexpr bool SB = ShortBatchKernel<U, GF, CMP, R>::value;
+    bool batch = false;
+    if constexpr (SB) batch = tiles_are_short<W, R>(rg, warp, lane, tb, Tc);
 #pragma unroll
     for (int kk = 0; kk < R; ++kk) {
         const int j = warp + kk * W;
@@ -714,11 +739,17 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_pipe(
         // K1: q = A w
         double qv[R];
         consumers_begin_pass(rg, pass);
+        if constexpr (SB) {
 #pragma unroll
-        for (int kk = 0; kk < R; ++kk) {
-            const int j = warp + kk * W;
-            qv[kk] = 0.0;
-            if (j < Tc) qv[kk] = consume_tile<U, false, CMP, GF>(rg, wpub[buf], pos, j, lane, (int)((tb + j) * kTileRows + lane));
+            for (int kk = 0; kk < R; ++kk) qv[kk] = 0.0;
+            k1_resident_tiles<W, U, R, CMP, GF>(rg, wpub[buf], pos, warp, lane, tb, Tc, batch, qv);
+        } else {
+#pragma unroll
+            for (int kk = 0; kk < R; ++kk) {
+                const int j = warp + kk * W;
+                qv[kk] = 0.0;
+                if (j < Tc) qv[kk] = consume_tile<U, false, CMP, GF>(rg, wpub[buf], pos, j, lane, (int)((tb + j) * kTileRows + lane));
+            }
         }
         ++pass; pos = ring_next_pass(rg, pos, Tc);
         CGS_STAMP(k, 1);

@@ -1,11 +1,23 @@
 // cg_variant.cu -- instantiates the kernels of ONE streamed kernel shape and ONE slot format.
-// Compiled six times (-DCG_SHAPE=0|1|2 -DCG_CMP=0|1) in parallel by build.py; nothing here but the
-// table of entry points (cg_variants.h).  The kernels themselves are in cg_stream_kernels.cuh.
+// Compiled six times (-DCG_SHAPE=0|1|2 -DCG_CMP=0|1) and once with -DCG_SHORT (the short-row kernels of
+// shape 2) in parallel by build.py; nothing here but the table of entry points (cg_variants.h).  The
+// kernels themselves are in cg_stream_kernels.cuh.
 #include "cg_stream_kernels.cuh"
 #include "cg_variants.h"
 
+#if defined(CG_SHORT)
+
+void cg_fill_fns_short(StreamFns& f) {
+    f.short_persistent[0] = (const void*)cgs::ks_persistent<16, 0, 9, true, 4, false, false, true>;
+    f.short_persistent[1] = (const void*)cgs::ks_persistent<16, 0, 9, true, 4, true, false, true>;
+    f.short_cg1 = (const void*)cgs::ks_persistent_cg1<16, 0, 9, true, 4, true>;
+    f.short_pipe = (const void*)cgs::ks_persistent_pipe<16, 0, 9, true, 4, true>;
+}
+
+#else
+
 #if !defined(CG_SHAPE) || !defined(CG_CMP)
-#error "compile with -DCG_SHAPE=0|1|2 -DCG_CMP=0|1"
+#error "compile with -DCG_SHAPE=0|1|2 -DCG_CMP=0|1, or -DCG_SHORT"
 #endif
 
 namespace {
@@ -55,3 +67,5 @@ void CG_FILL_NAME(CG_SHAPE, CG_CMP)(StreamFns& f) {
     fill<16, 0, 27, true, CG_CMP != 0>(f);
 #endif
 }
+
+#endif  // CG_SHORT

@@ -17,8 +17,14 @@ struct StreamFns {
     const void* persistent[2][kNumPersistent];
     const void* cg1[2][2];                 // option "algo" = 1 (Chronopoulos-Gear): [cmp][R == 4]
     const void* pipe[2][2];                // option "algo" = 2 (pipelined CG); null for shape 0
+    // Short-row kernels (shape 2, compressed index, no row longer than 9 entries, 4 rows per thread): U = 9 and
+    // several tiles' gathers in flight per warp (cg_stream.cuh: short_batch).  Null for the other shapes.
+    const void* short_persistent[2];       // [Jacobi]
+    const void* short_cg1;
+    const void* short_pipe;
 };
 
 void cg_fill_fns_0_0(StreamFns&); void cg_fill_fns_0_1(StreamFns&);
 void cg_fill_fns_1_0(StreamFns&); void cg_fill_fns_1_1(StreamFns&);
 void cg_fill_fns_2_0(StreamFns&); void cg_fill_fns_2_1(StreamFns&);
+void cg_fill_fns_short(StreamFns&);      // cg_variant.cu compiled with -DCG_SHORT

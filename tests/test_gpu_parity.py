@@ -550,6 +550,38 @@ def test_ring_and_grid_options_same_bits(bound):
     B.cg.set_option("spmv", 0)
 
 
+@pytest.mark.parametrize("grid", [None, 50, 45])
+def test_short_row_kernels_same_bits(bound, orc, grid):
+    """The short-row kernels ("short_rows", chosen when no row has more than 9 entries: the 7-point
+    Laplacian) keep the gathers of several tiles in flight per warp; per row the operations and their
+    order are those of the one-tile trip, so the bits of every loop (textbook, Jacobi, Chronopoulos-Gear,
+    pipelined) are those of the kernels they replace.  64^3 (config 1: 3 or 4 tiles per warp), 50^3 (a ragged
+    last tile, which falls back to the one-tile trip) and 45^3 (1 or 2 tiles per warp); parity against the
+    oracle on top."""
+    B = bound(1, grid)
+    p = B.p
+    for name, v in (("loop", 0), ("spmv", 0), ("fold", 2), ("algo", 0), ("short_rows", 1)):
+        B.cg.set_option(name, v)
+    assert B.cg.info("spmv") == 4 and B.cg.info("short_rows") == 1 and B.cg.info("fold") == 0
+    ref = oracle_solve(orc, p, ("cfg1", grid))
+    for algo, jacobi in ((0, False), (0, True), (1, False), (2, False)):
+        B.cg.set_option("algo", algo)
+        runs = []
+        for short in (1, 0):
+            B.cg.set_option("short_rows", short)
+            B.cg.set_option("fold", 0)                  # short_rows = 0 alone would fold (auto), other bits
+            assert B.cg.info("short_rows") == short
+            x, res = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit, jacobi=jacobi)
+            runs.append((x, res))
+        (x1, r1), (x0, r0) = runs
+        assert r1.iters == r0.iters and r1.status == r0.status
+        assert torch.equal(r1.hist, r0.hist) and torch.equal(x1, x0), (algo, jacobi)
+        if not jacobi:                                  # (the diagonal is constant: Jacobi is CG on a scaled system)
+            check_solve_parity(r1, x1, ref)
+    for name, v in (("algo", 0), ("fold", 2), ("short_rows", 1)):
+        B.cg.set_option(name, v)
+
+
 @pytest.mark.parametrize("ctas", [1, 2, 3])
 def test_generic_ctas_per_sm(bound, orc, ctas):
     B = bound(0)
