@@ -247,7 +247,10 @@ int cg_probe_grid_sync(cg_handle* h, int kind, int reps, double* h_cycles, void*
  * barrier.  Layout [cta][iter][slot]; row `iters` of every CTA holds ring statistics
  * ([0] cycles producer warp 0 waited for free slots, [1] its lifetime, [2] tiles it issued,
  * [3] cycles consumer thread 0 waited for data).  NULL or iters = 0 switches it off (the
- * default).  The buffer is borrowed. */
+ * default).  The buffer is borrowed.  With cg_set_option "trace_clock" = 1 the streamed
+ * persistent kernels stamp %globaltimer (nanoseconds, one clock for all SMs) instead, which
+ * makes the stamps of different CTAs comparable: arrival and release skew at each grid
+ * synchronisation. */
 int cg_set_trace(cg_handle* h, uint64_t* d_trace, int64_t iters);
 
 /* Frees the host struct (and any CUDA graph).  Device memory is the caller's. */

@@ -481,7 +481,7 @@ struct cg_handle {
     unsigned char* idx; size_t idx_bytes; bool idx_ready; int idx_codes;     // compressed index (borrowed buffer)
     cudaGraphExec_t gexec; int gexec_variant, gexec_chunk, gexec_grid, gexec_cmp; size_t gexec_smem;
     cudaStream_t cap_stream;               // capture-only stream (the legacy stream cannot capture)
-    unsigned long long* trace; int trace_iters;
+    unsigned long long* trace; int trace_iters, trace_clock;
     long long launches;
     int last_resident, last_fold, last_short;      // what the last persistent solve used (info)
     int last_chk_errors;                   // violations counted by the last checked cg_spmv
@@ -666,7 +666,7 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     P->part0 = h->part0; P->part1 = h->part1; P->part2 = h->part2; P->part3 = h->part3;
     P->scal = h->scal; P->hist = hist; P->rtol = rtol; P->maxit = maxit;
     P->precond = precond; P->spmv = variant; P->tpr = h->tpr;
-    P->trace = h->trace; P->trace_iters = h->trace_iters;
+    P->trace = h->trace; P->trace_iters = h->trace_iters; P->trace_clock = h->trace_clock;
     P->rp_pad = h->rp_pad; P->bslots = h->bslots;
     P->cap = g.cap; P->slots = g.slots; P->slot_bytes = g.slot_bytes;
     P->pinned = g.pinned; P->stream_slots = g.stream_slots;
@@ -885,6 +885,7 @@ extern "C" int cg_set_option(cg_handle* h, const char* name, int64_t value) {
     if (!strcmp(name, "smem_cap_kb")) { if (value < 0 || value > 227) return CG_EINVAL; h->smem_cap_kb = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
+    if (!strcmp(name, "trace_clock")) { if (value < 0 || value > 1) return CG_EINVAL; h->trace_clock = (int)value; return CG_OK; }
     if (!strcmp(name, "short_rows")) { if (value < 0 || value > 1) return CG_EINVAL; h->short_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "spin_budget_ms")) { if (value < 1 || value > 600000) return CG_EINVAL; h->spin_budget_ms = (int)value; return CG_OK; }

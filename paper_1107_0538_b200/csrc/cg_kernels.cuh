@@ -81,6 +81,7 @@ struct Params {
     int tpr;              // lanes per row of the vector variant
     unsigned long long* trace;   // optional phase stamps of the persistent kernel (cg_set_trace)
     int trace_iters;
+    int trace_clock;             // 0: clock64 (SM cycles, per SM); 1: %globaltimer (ns, one clock for all SMs)
     // streamed variants (cg_stream.cuh)
     const int* rp_pad;    // rowptr copied into the workspace, padded with nnz (bulk copies of 36 ints)
     double* bslots;       // grid all-reduce inboxes [cta][3][kBarVals][kBarGrid], all-ones when idle

@@ -171,6 +171,12 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks3_update_p(const 
 // grid_allreduce's slot recycling needs a fully fenced synchronisation strictly between any
 // all-reduce and the third all-reduce after it (see cg_stream.cuh); plan_is_safe checks that
 // for the cyclic sequence, and the call sites below take their kind from the plan.
+// Time stamp of the phase trace: SM cycles, or (option "trace_clock" = 1) the nanosecond clock all SMs share,
+// which makes stamps of different CTAs comparable (arrival and release skew at the grid synchronisations).
+__device__ __forceinline__ unsigned long long trace_now(const Params& P) {
+    if (P.trace_clock) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+    return (unsigned long long)clock64();
+}
 enum SyncKind { kArRelaxed = 0, kArFenced = 1, kCounter = 2 };
 template <bool FOLD> struct SyncPlan;
 template <> struct SyncPlan<false> { static constexpr int n = 3; static constexpr SyncKind seq[3] = {kArRelaxed, kArRelaxed, kCounter}; };
@@ -295,7 +301,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent(Param
     // with beta = 0, for which fma(beta, p, r) is r = p_0 to the bit.
     double beta_prev = 0.0;
     int cur = 0;
-#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
+#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = trace_now(P); } while (0)
     while (!stop) {
         CGS_STAMP(k, 0);
         // K1: q = A p, partial p.q
@@ -524,7 +530,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
     }
     unsigned long long* tr = (P.trace && threadIdx.x == 0)
         ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
-#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
+#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = trace_now(P); } while (0)
     while (!stop) {
         // trace slots of this loop, in order: 0 pass start, 1 vector updates done, 2 past the publish
         // barrier, 3 K1 done, 4 past the all-reduce, 5 = 6 = 7 scalars done
@@ -733,7 +739,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_pipe(
     if (dead) { stop = 1; status = CG_ETIMEOUT; }
     unsigned long long* tr = (P.trace && threadIdx.x == 0)
         ? P.trace + (size_t)cta * (P.trace_iters + 1) * kTraceSlots : nullptr;
-#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = clock64(); } while (0)
+#define CGS_STAMP(it, slot) do { if (tr && (it) < P.trace_iters) tr[(it) * kTraceSlots + (slot)] = trace_now(P); } while (0)
     while (!stop) {
         CGS_STAMP(k, 0);
         // K1: q = A w
