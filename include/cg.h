@@ -23,7 +23,8 @@
  *    Columns of a row need not be sorted or unique (duplicates add).
  *  - Return codes: 0 success / converged.  Positive = soft outcome: of cg_solve
  *    1 maxit reached, 2 breakdown (p.Ap <= 0 or not finite: A is not SPD); of
- *    cg_compress_index 3 (the index was left uncompressed).
+ *    cg_compress_index 3 (the index was left uncompressed); of cg_reorder 4 (the matrix
+ *    was left in the caller's numbering).
  *    Negative = error: -1 invalid argument, -2 CUDA error (text via
  *    cg_strerror), -3 device not supported (needs compute capability 10.x),
  *    -4 device watchdog (a spin wait inside a solve ran out of its budget: a
@@ -51,6 +52,7 @@ typedef struct cg_handle cg_handle;
 #define CG_MAXIT          1
 #define CG_BREAKDOWN      2
 #define CG_NOTCOMPRESSED  3
+#define CG_NOTREORDERED   4
 #define CG_EINVAL        -1
 #define CG_ECUDA         -2
 #define CG_EUNSUPPORTED  -3
@@ -87,6 +89,30 @@ int cg_create(cg_handle** out, int64_t n, int64_t nnz,
  * changes) or a negative error.  Synchronises the stream. */
 size_t cg_index_bytes(cg_handle* h);
 int cg_compress_index(cg_handle* h, void* d_index, size_t index_bytes, void* cuda_stream);
+
+/* Optional renumbering for matrices whose rows arrive in no useful order (the
+ * matrix comes from a FEM model of an electrical machine, numbered as the mesh generator left
+ * it; BASELINE.json config 3).  When one warp-wide gather of the SpMV touches many 128-byte
+ * lines (cg_get_info "lines_per_gather_x100"), K1 is bound by the 32-byte sectors the L2 has to
+ * deliver for 8 useful bytes each.  cg_reorder computes a reverse Cuthill-McKee numbering on
+ * the host (the pattern is copied there once; set-up work, like cg_create), builds the matrix
+ * P A P^T in caller-owned device memory (entries of a row sorted by their new column) and binds
+ * an inner handle to it.  From then on cg_solve / cg_solve_jacobi / cg_solve_host gather b and
+ * x0 into the new numbering, run the SAME kernels on the renumbered matrix and scatter x back:
+ * two small extra launches per solve, iterates equal to the caller's up to the rounding of a
+ * different summation order (same parity bands in the tests).  cg_spmv, cg_dot and
+ * cg_check_csr keep using the caller's matrix.  Options set later reach both handles;
+ * "values_changed" drops the renumbered copy (call cg_reorder again); "reorder" = 0 / 1
+ * switches its use off / on.
+ * cg_reorder_bytes: size of d_buf (permutation, the renumbered CSR arrays, two vectors, the
+ * inner handle's workspace).  cg_reorder: d_buf 256-byte aligned, borrowed until cg_destroy or
+ * the next call; returns CG_OK (in use from now on), CG_NOTREORDERED (the new numbering
+ * does not cut the lines per gather by at least a third: nothing changes) or a negative
+ * error.  Synchronises the stream.
+ * cg_rcm_host: the numbering alone, host arrays in, h_perm[new row] = old row out. */
+size_t cg_reorder_bytes(int64_t n, int64_t nnz);
+int cg_reorder(cg_handle* h, void* d_buf, size_t bytes, void* cuda_stream);
+int cg_rcm_host(int64_t n, const int32_t* h_rowptr, const int32_t* h_colind, int32_t* h_perm);
 
 /* Optional structural check of the bound CSR arrays on the device: rowptr[0] = 0,
  * rowptr[n] = nnz, non-decreasing, 0 <= colind < n.  Synchronises the stream.
@@ -213,9 +239,11 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
  * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "pinned_tiles", "slot_bytes",
- * "resident_rows", "fold", "short_rows", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
+ * "reordered" (cg_reorder's numbering is in use), "resident_rows", "fold", "short_rows", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
  * counted by the last checked cg_spmv), "lines_per_gather_x100"
  * (cg_create statistic: 128-byte lines one warp-wide gather touches on average, times 100).
+ * A name prefixed with "solve_" ("solve_spmv", "solve_ring_slots", ...) is answered by the handle
+ * the solves run on: the renumbered one after cg_reorder, this one otherwise.
  * Unknown names return CG_EINVAL. */
 int cg_set_option(cg_handle* h, const char* name, int64_t value);
 int cg_get_info(cg_handle* h, const char* name, int64_t* value);

@@ -26,6 +26,9 @@ SIGNATURES = {
     "cg_create": (ctypes.c_int, [ctypes.POINTER(_vp), _i64, _i64, _vp, _vp, _vp, _vp, _sz]),
     "cg_index_bytes": (_sz, [_vp]),
     "cg_compress_index": (ctypes.c_int, [_vp, _vp, _sz, _vp]),
+    "cg_reorder_bytes": (_sz, [_i64, _i64]),
+    "cg_reorder": (ctypes.c_int, [_vp, _vp, _sz, _vp]),
+    "cg_rcm_host": (ctypes.c_int, [_i64, _vp, _vp, _vp]),
     "cg_check_csr": (ctypes.c_int, [_vp, _vp]),
     "cg_spmv": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "cg_dot": (ctypes.c_int, [_vp, _vp, _vp, ctypes.POINTER(_f64), _vp]),
@@ -108,6 +111,25 @@ def cg_compress_index(h: int, d_index: int, index_bytes: int, stream: int = 0) -
     if rc < 0:
         raise CGError(rc, "cg_compress_index")
     return rc
+
+
+def cg_reorder_bytes(n: int, nnz: int) -> int:
+    return int(lib().cg_reorder_bytes(n, nnz))
+
+
+def cg_reorder(h: int, d_buf: int, nbytes: int, stream: int = 0) -> int:
+    """Returns 0 (solves now run on the renumbered matrix) or 4 (CG_NOTREORDERED); raises on errors."""
+    rc = lib().cg_reorder(h, d_buf, nbytes, stream)
+    if rc < 0:
+        raise CGError(rc, "cg_reorder")
+    return rc
+
+
+def cg_rcm_host(n: int, h_rowptr: int, h_colind: int, h_perm: int) -> None:
+    """Host arrays (raw addresses): int32 rowptr[n+1], colind[nnz] in, int32 perm[n] out."""
+    rc = lib().cg_rcm_host(n, h_rowptr, h_colind, h_perm)
+    if rc != 0:
+        raise CGError(rc, "cg_rcm_host")
 
 
 def cg_check_csr(h: int, stream: int = 0) -> int:
@@ -208,7 +230,7 @@ class CGResult:
 class CG:
     """Handle bound to CSR arrays held in torch CUDA tensors (kept alive here)."""
 
-    def __init__(self, rowptr, colind, vals, compress: bool = True):
+    def __init__(self, rowptr, colind, vals, compress: bool = True, reorder: bool = True):
         import torch
         if not (rowptr.is_cuda and colind.is_cuda and vals.is_cuda):
             raise ValueError("CSR arrays must be CUDA tensors (there is no CPU path)")
@@ -226,8 +248,13 @@ class CG:
                            self.vals.data_ptr(), self.workspace.data_ptr(), wb)
         self._scratch = None
         self.index = None
+        self.renumbered = None
         if compress:
             self.compress()
+        # irregular gathers (more than 8 lines per warp-wide gather, the library's own threshold for
+        # "irregular"): let the library renumber the matrix for the solves
+        if reorder and self.info("lines_per_gather_x100") > 800:
+            self.reorder()
 
     def compress(self) -> bool:
         """Build the compressed column index (cg_compress_index) in a tensor owned here.
@@ -238,6 +265,15 @@ class CG:
         buf = self.torch.empty(nb, dtype=self.torch.uint8, device=self.device)
         rc = cg_compress_index(self.h, buf.data_ptr(), nb, self._stream())
         self.index = buf if rc == 0 else None
+        return rc == 0
+
+    def reorder(self) -> bool:
+        """Reverse Cuthill-McKee renumbering for the solves (cg_reorder) in a tensor owned here.
+        Returns True when the handle now solves on the renumbered matrix."""
+        nb = cg_reorder_bytes(self.n, self.nnz)
+        buf = self.torch.empty(nb, dtype=self.torch.uint8, device=self.device)
+        rc = cg_reorder(self.h, buf.data_ptr(), nb, self._stream())
+        self.renumbered = buf if rc == 0 else None
         return rc == 0
 
     def close(self):

@@ -1,7 +1,7 @@
 """Build libcg_b200.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo).
 
 cg_api.cu (ABI, setup kernels, generic path) and seven instances of cg_variant.cu (one per streamed
-kernel shape and slot format, one for the short-row kernels) are compiled in parallel and linked into one shared library."""
+kernel shape and slot format, one for the short-row kernels) and cg_rcm.cpp (host-side renumbering) are compiled in parallel and linked into one shared library."""
 from __future__ import annotations
 
 import os
@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "cg_api.cu"), os.path.join(CSRC, "cg_variant.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("cg_kernels.cuh", "cg_stream.cuh", "cg_stream_kernels.cuh", "cg_variants.h")] \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("cg_kernels.cuh", "cg_stream.cuh", "cg_stream_kernels.cuh", "cg_variants.h", "cg_rcm.cpp")] \
     + [os.path.join(ROOT, "include", "cg.h")]
 LIB = os.path.join(HERE, "libcg_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
@@ -42,6 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         units = [("api", SOURCES[0], [])]
         units += [(f"shape{s}_cmp{c}", SOURCES[1], [f"-DCG_SHAPE={s}", f"-DCG_CMP={c}"]) for s in range(3) for c in range(2)]
         units += [("short", SOURCES[1], ["-DCG_SHORT"])]
+        units += [("rcm", os.path.join(CSRC, "cg_rcm.cpp"), [])]
         procs = []
         for name, src, defs in units:
             obj = os.path.join(tmp, name + ".o")
