@@ -120,22 +120,30 @@ def whole_job_value(dist, device, iterations_this_rank, seconds_this_rank):
 
 
 def describe(A):
-    """Launch configuration of a bound handle, from cg_get_info."""
-    v = A.info("spmv")
-    d = {"loop": {0: "persistent cooperative kernel", 1: "cuda graph", 2: "stepwise launches"}[A.info("loop")],
-         "grid": A.info("grid"), "block": A.info("block"), "smem_bytes": A.info("smem")}
+    """Launch configuration of the handle the solves run on, from cg_get_info ("solve_*": the renumbered
+    matrix's handle after cg_reorder, else the handle itself)."""
+    info = lambda name: A.info("solve_" + name)
+    v = info("spmv")
+    d = {"loop": {0: "persistent cooperative kernel", 1: "cuda graph", 2: "stepwise launches"}[info("loop")],
+         "grid": info("grid"), "block": info("block"), "smem_bytes": info("smem")}
+    if A.info("reordered"):
+        d["numbering"] = (f"reverse Cuthill-McKee (cg_reorder): {A.info('lines_per_gather_x100') / 100:.1f} -> "
+                          f"{info('lines_per_gather_x100') / 100:.1f} lines per warp-wide gather; b, x0 gathered and x "
+                          "scattered by two small kernels inside the timed region")
     if v == 1:
-        d["spmv"] = f"generic: {A.info('tpr')} lanes per row from global memory"
+        d["spmv"] = f"generic: {info('tpr')} lanes per row from global memory"
     else:
-        npw, pin, slots = A.info("producer_warps"), A.info("pinned_tiles"), A.info("ring_slots")
-        who = (f"{npw} TMA producer warps + {A.info('consumer_warps')} consumer warps" if npw
-               else f"{A.info('consumer_warps')} consumer warps, each copying its own tiles once per launch (TMA bulk copies)")
-        where = (f"{slots} x {A.info('slot_bytes')} B tiles pinned in shared memory" if pin >= slots
-                 else f"ring of {slots} x {A.info('slot_bytes')} B tiles" + (f", {pin} of them pinned" if pin else ""))
-        d["spmv"] = (f"streamed: {who}, one lane per row, {A.info('in_flight')} gathers in flight per lane, {where}, "
-                     + ("compressed column index (9 B per entry)" if A.info("compressed") else "plain CSR slots (12 B per entry)"))
-        rr = A.info("resident_rows")
-        d["vectors"] = (f"x, r, p, q in registers ({rr} rows per thread)" if rr and A.info("loop") == 0
+        npw, pin, slots = info("producer_warps"), info("pinned_tiles"), info("ring_slots")
+        who = (f"{npw} TMA producer warps + {info('consumer_warps')} consumer warps" if npw
+               else f"{info('consumer_warps')} consumer warps, each copying its own tiles once per launch (TMA bulk copies)")
+        where = (f"{slots} x {info('slot_bytes')} B tiles pinned in shared memory" if pin >= slots
+                 else f"ring of {slots} x {info('slot_bytes')} B tiles" + (f", {pin} of them pinned" if pin else ""))
+        flight = ("9 gathers per tile, 2-3 tiles in flight per lane (short-row kernel)" if info("short_rows")
+                  else f"{info('in_flight')} gathers in flight per lane")
+        d["spmv"] = (f"streamed: {who}, one lane per row, {flight}, {where}, "
+                     + ("compressed column index (9 B per entry)" if info("compressed") else "plain CSR slots (12 B per entry)"))
+        rr = info("resident_rows")
+        d["vectors"] = (f"x, r, p, q in registers ({4 if info('short_rows') else rr} rows per thread)" if rr and info("loop") == 0
                         else "x, r, p, q in global memory")
     return d
 
@@ -148,10 +156,14 @@ def workload_string(p):
 
 def kernel_name(A):
     """Which instantiation of the persistent kernel a handle launches, from cg_get_info."""
-    if A.info("spmv") == 1:
+    info = lambda name: A.info("solve_" + name)
+    if info("spmv") == 1:
         return "k_persistent (generic)"
-    return (f"ks_persistent<W={A.info('consumer_warps')},NP={A.info('producer_warps')},U={A.info('in_flight')},"
-            f"R={A.info('resident_rows')},fold={A.info('fold')},cmp={A.info('compressed')}>")
+    if info("short_rows"):
+        return f"ks_persistent<W={info('consumer_warps')},NP=0,U=9,R=4,fold=0,cmp=1> (short rows)"
+    return (f"ks_persistent<W={info('consumer_warps')},NP={info('producer_warps')},U={info('in_flight')},"
+            f"R={info('resident_rows')},fold={info('fold')},cmp={info('compressed')}>"
+            + (" (renumbered)" if A.info("reordered") else ""))
 
 
 def traffic_entry(cfg, kernel, iterations):
@@ -213,7 +225,7 @@ def per_config_leg(cg, torch, dev, cfg, p, args, peak, l2_gbs, flush_l2, with_cp
         "roofline": {"bound": "hbm", "achieved": bytes_it / med / 1e9, "peak": peak, "unit": "GB/s",
                      "frac": bytes_it / med / 1e9 / peak,
                      "bytes_model": "12 NNZ + 92 N + 4 per iteration (SURVEY.md 8(d): plain CSR, the method's bytes)"
-                                    + ("; the compressed index moves 9.1 NNZ + 92 N" if A.info("compressed") else ""),
+                                    + ("; the compressed index moves 9.1 NNZ + 92 N" if A.info("solve_compressed") else ""),
                      **traffic_entry(cfg, kernel_name(A), K)},
         "launch": describe(A),
     }
@@ -238,7 +250,7 @@ def per_config_leg(cg, torch, dev, cfg, p, args, peak, l2_gbs, flush_l2, with_cp
                    "what": f"cg_spmv, {reps} back-to-back launches (each one refills its shared-memory slots"
                            + (" from the L2" if cfg != 4 else " from HBM") + ")"}
     # K1 inside the persistent loop, from the phase trace (slowest CTA per iteration)
-    if A.info("loop") == 0 and A.info("spmv") >= 2:
+    if A.info("loop") == 0 and A.info("solve_spmv") >= 2:
         n_tr = 24
         tr = A.trace(n_tr)
         timed_solve(0.0, n_tr, False)
@@ -259,7 +271,7 @@ def per_config_leg(cg, torch, dev, cfg, p, args, peak, l2_gbs, flush_l2, with_cp
         var = {}
         for algo, name in ((1, "chronopoulos_gear"), (2, "pipelined")):
             A.set_option("algo", algo)
-            if A.info("algo") == algo:
+            if A.info("solve_algo") == algo:
                 timed_solve(p.rtol, p.maxit, True)
                 runs = sorted((timed_solve(p.rtol, p.maxit, True) for _ in range(3)), key=lambda r: r[0])
                 t, it, st = runs[1]
@@ -268,6 +280,16 @@ def per_config_leg(cg, torch, dev, cfg, p, args, peak, l2_gbs, flush_l2, with_cp
                              "what": "solve to convergence, prologue (two SpMVs) included"}
         A.set_option("algo", 0)
         rec["reduced_sync_variants"] = var
+    if A.info("reordered"):
+        # the same fixed work in the caller's numbering: the gather-bound regime the config stands for
+        A.set_option("reorder", 0)
+        timed_solve(0.0, K, False)
+        t0s = [timed_solve(0.0, K, True)[0] / K for _ in range(3)]
+        m0 = float(np.median(t0s))
+        rec["callers_numbering"] = {"us_per_iteration": m0 * 1e6, "frac_of_hbm_roofline": bytes_it / m0 / 1e9 / peak,
+                                    "launch": describe(A), **traffic_entry(cfg, kernel_name(A), K),
+                                    "what": 'cg_set_option "reorder" = 0: same handle, same kernels, rows as the caller numbered them'}
+        A.set_option("reorder", 1)
     if cfg != 4:
         timed_solve(p.rtol, p.maxit, True)
         tc = [timed_solve(p.rtol, p.maxit, True) for _ in range(3)]
@@ -381,6 +403,10 @@ def main():
     ap.add_argument("--pin", type=int, default=None)
     ap.add_argument("--compress", type=int, default=None)
     ap.add_argument("--algo", type=int, default=None, help="with --profile: 1 = Chronopoulos-Gear, 2 = pipelined CG")
+    ap.add_argument("--reorder", type=int, default=None, help="with --profile: 0 = solve in the caller's numbering")
+    ap.add_argument("--short-rows", type=int, default=None, dest="short_rows", help="with --profile: 0 = no short-row kernels")
+    ap.add_argument("--trace-clock", type=int, default=0, dest="trace_clock",
+                    help="with --trace: 1 = stamp %%globaltimer (ns, comparable across CTAs) and print the skew at each synchronisation")
     ap.add_argument("--trace", action="store_true",
                     help="with --profile and --loop 0: print the per-phase cycle breakdown (cg_set_trace)")
     args = ap.parse_args()
@@ -447,9 +473,14 @@ def main():
             Ap.set_option("compress", args.compress)
         if args.algo is not None:
             Ap.set_option("algo", args.algo)
+        if args.reorder is not None:
+            Ap.set_option("reorder", args.reorder)
+        if args.short_rows is not None:
+            Ap.set_option("short_rows", args.short_rows)
         bp = torch.from_numpy(pp.b).to(dev)
         xp = torch.zeros(pp.n, dtype=torch.float64, device=dev)
         out = []
+        Ap.set_option("trace_clock", args.trace_clock)
         tr = Ap.trace(args.profile_iters) if (args.trace and args.loop == 0) else None
         for rep in range(3):
             xp.zero_()
@@ -462,9 +493,11 @@ def main():
             torch.cuda.synchronize()
             out.append(e0.elapsed_time(e1) * 1e3 / max(it, 1))
         rec = {"profile_config": args.profile, "iters": args.profile_iters, "us_per_iteration": out,
-               "loop": Ap.info("loop"), "spmv": Ap.info("spmv"), "grid": Ap.info("grid"),
-               "compressed": Ap.info("compressed"), "pinned_tiles": Ap.info("pinned_tiles"),
-               "ring_slots": Ap.info("ring_slots"), "fold": Ap.info("fold"), "resident_rows": Ap.info("resident_rows"), "algo": Ap.info("algo")}
+               "loop": Ap.info("solve_loop"), "spmv": Ap.info("solve_spmv"), "grid": Ap.info("solve_grid"),
+               "compressed": Ap.info("solve_compressed"), "pinned_tiles": Ap.info("solve_pinned_tiles"),
+               "ring_slots": Ap.info("solve_ring_slots"), "fold": Ap.info("solve_fold"), "resident_rows": Ap.info("solve_resident_rows"),
+               "algo": Ap.info("solve_algo"), "short_rows": Ap.info("solve_short_rows"), "reordered": Ap.info("reordered"),
+               "kernel": kernel_name(Ap)}
         if tr is not None:
             # [cta, iter, slot] clock64 stamps -> cycles per interval; skip the first 2 iterations
             full = tr.cpu().numpy().astype(np.int64)
@@ -474,7 +507,7 @@ def main():
             t = full[:, 2:args.profile_iters - 1, :]
             names = {0: ["K1 work", "barrier 1", "alpha + K2 work", "barrier 2", "beta", "K3 work", "barrier 3"],
                      1: ["vector updates", "publish barrier", "K1 work", "all-reduce", "scalars", "(unused a)", "(unused b)"],
-                     2: ["K1 work", "partials read + sum", "scalars", "(unused a)", "(unused b)", "vector updates", "barrier"]}[Ap.info("algo")]
+                     2: ["K1 work", "partials read + sum", "scalars", "(unused a)", "(unused b)", "vector updates", "barrier"]}[Ap.info("solve_algo")]
             d = np.diff(t[:, :, :8], axis=2)
             if t.shape[2] >= 16 and t[:, :, 8:].any():
                 dd = np.diff(t[:, :, 8:], axis=2)
@@ -483,6 +516,20 @@ def main():
             rec["trace_cycles"] = {nm: {"mean": float(d[:, :, i].mean()), "max_cta": float(d[:, :, i].max(axis=0).mean()),
                                         "min_cta": float(d[:, :, i].min(axis=0).mean())} for i, nm in enumerate(names)}
             rec["trace_cycles"]["iteration"] = float((t[:, :, 7] - t[:, :, 0]).mean())
+            if args.trace_clock:
+                # one clock for all SMs: the stamps of different CTAs can be compared.  Per synchronisation of the
+                # textbook loop: how far apart the CTAs arrive, and how long after the LAST arrival the first, the
+                # average and the last CTA leave (nanoseconds, means over the iterations).
+                rec["trace_unit"] = "ns (%globaltimer)"
+                g = (t[:, :, :8] - t[:, :, :8].min()).astype(np.float64)      # int64 first: 1.7e18 ns does not fit a double's 53 bits
+                sk = {}
+                for a, b_, nm in ((1, 2, "sync 1"), (3, 4, "sync 2"), (6, 7, "sync 3")):
+                    last_in = g[:, :, a].max(axis=0)
+                    sk[nm] = {"arrival_spread": float((last_in - g[:, :, a].min(axis=0)).mean()),
+                              "last_arrival_to_first_release": float((g[:, :, b_].min(axis=0) - last_in).mean()),
+                              "last_arrival_to_mean_release": float((g[:, :, b_].mean(axis=0) - last_in).mean()),
+                              "last_arrival_to_last_release": float((g[:, :, b_].max(axis=0) - last_in).mean())}
+                rec["sync_skew_ns"] = sk
         print(json.dumps(rec))
         Ap.close()
         return

@@ -61,15 +61,17 @@ typedef struct cg_handle cg_handle;
 
 /* Bytes of device workspace cg_create needs for an n-row system: the vectors
  * r, p, q, one spare and D^-1 (each n doubles, 256-byte aligned), a padded copy of rowptr
- * (n + 41 ints), the per-CTA reduction partials, the grid all-reduce inboxes (1.8 MB) and
- * the device-resident scalar state. */
+ * (n + 41 ints), the per-CTA reduction partials, a 16 MB reserve inside which the grid
+ * all-reduce inboxes (1.8 MB) are placed, and the device-resident scalar state. */
 size_t cg_workspace_bytes(int64_t n);
 
 /* Bind a handle to a CSR matrix already resident on the device.
  * d_rowptr int32[n+1], d_colind int32[nnz], d_vals double[nnz].
  * d_workspace: >= cg_workspace_bytes(n) bytes, 256-byte aligned.
  * Reads the n+1 row pointers once (two stream-0 kernels: tile statistics, padded copy) to
- * pick the SpMV variant and the ring geometry.
+ * pick the SpMV variant and the ring geometry, and times the grid synchronisation with the
+ * all-reduce inboxes at 40 places of their reserve (which L2 slices their lines map to
+ * changes its cost by a few per cent; ~30 ms; results never depend on the place).
  * Errors: CG_EINVAL on NULL/misaligned pointers, n <= 0, nnz < 0, n or nnz
  * >= 2^31, workspace too small; CG_EUNSUPPORTED off sm_100; CG_ECUDA. */
 int cg_create(cg_handle** out, int64_t n, int64_t nnz,
@@ -194,6 +196,8 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               instead of three times per iteration; 0 = off; 2 (default) = on when a CTA
  *               gathers <= 500 entries per lane-row set (tiles x mean row length) and the
  *               short-row kernels do not apply
+ *   "sync_place" where the all-reduce inboxes sit in their reserve, in steps of 64 KB
+ *               (0 .. cg_get_info "sync_places"); cg_create picks it by measurement
  *   "short_rows" 1 (default) = when no row has more than 9 entries (the 7-point Laplacian), every
  *               CTA's slice is pinned and a consumer warp owns several tiles, run the kernels
  *               that keep the gathers of 2-3 tiles in flight per warp instead of one tile's 9
@@ -239,7 +243,7 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  * cg_get_info reads back: "loop", "spmv", "grid", "block", "smem", "launches" (kernels
  * launched by the last call), "sms", "tpr", "max_row_len", "max_tile_nnz", "stream_ok",
  * "consumer_warps", "producer_warps", "in_flight", "ring_slots", "pinned_tiles", "slot_bytes",
- * "reordered" (cg_reorder's numbering is in use), "resident_rows", "fold", "short_rows", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
+ * "sync_place", "sync_places", "reordered" (cg_reorder's numbering is in use), "resident_rows", "fold", "short_rows", "algo", "compressed", "index_codes", "from_hbm", "check_errors" (violations
  * counted by the last checked cg_spmv), "lines_per_gather_x100"
  * (cg_create statistic: 128-byte lines one warp-wide gather touches on average, times 100).
  * A name prefixed with "solve_" ("solve_spmv", "solve_ring_slots", ...) is answered by the handle

@@ -466,6 +466,7 @@ struct cg_handle {
     const int* rowptr; const int* colind; const double* vals;
     unsigned char* ws; size_t ws_bytes;
     double *r, *p, *q, *dinv, *spare, *part0, *part1, *part2, *part3, *bslots;
+    unsigned char* bslots_base; int sync_place;
     int* rp_pad;
     Scal* scal; Params* dparams;
     Scal* h_scal; Params* h_params;        // pinned host mirrors
@@ -501,10 +502,15 @@ static constexpr int kNumVecs = 5;
 static constexpr size_t kPartBytes = (size_t)kMaxGrid * 8u;
 static constexpr size_t kBslotBytes = (size_t)cgs::kInboxStride * cgs::kBarGrid * 8u;    // one inbox per CTA
 static constexpr size_t kScalBytes = 512, kParamBytes = 512;
+// The all-reduce inboxes may sit anywhere in a reserve of 16 MB (option "sync_place", in steps of 64 KB): which
+// L2 slices and which die their lines map to changes the cost of a grid all-reduce by ~4 % (measured), so
+// cg_create tries a few places and keeps the fastest.
+static constexpr size_t kBslotStep = 64u << 10, kBslotReserve = 16u << 20;
+static constexpr int kBslotPlaces = (int)((kBslotReserve - kBslotBytes) / kBslotStep);
 
 extern "C" size_t cg_workspace_bytes(int64_t n) {
     if (n <= 0) return 0;
-    return kNumVecs * vec_bytes(n) + rp_pad_bytes(n) + 4 * kPartBytes + kBslotBytes + kScalBytes + kParamBytes;
+    return kNumVecs * vec_bytes(n) + rp_pad_bytes(n) + 4 * kPartBytes + kBslotReserve + kScalBytes + kParamBytes;
 }
 
 extern "C" size_t cg_host_scratch_bytes(int64_t n, int64_t maxit) {
@@ -688,6 +694,26 @@ static void fill_params(const cg_handle* h, Params* P, const double* b, double* 
     P->inject_fault = h->inject_fault;
 }
 
+// Where the all-reduce inboxes go is decided by measurement (see kBslotReserve): the mixed sequence of the
+// textbook loop {all-reduce, all-reduce, counter barrier} is timed at kTunePlaces places, the fastest kept.
+// ~30 ms of cg_create; results never depend on the place (the sums have one fixed order).
+static constexpr int kTunePlaces = 40, kTuneReps = 400;
+static int tune_sync_place(cg_handle* h) {
+    if (h->sms > cgs::kBarGrid) return CG_OK;
+    int best = 0; double best_c = 0.0;
+    for (int k = 0; k < kTunePlaces && k <= kBslotPlaces; ++k) {
+        h->bslots = reinterpret_cast<double*>(h->bslots_base + (size_t)k * kBslotStep);
+        double c = 0.0;
+        const int rc = cg_probe_grid_sync(h, 1, kTuneReps, &c, nullptr);
+        if (rc != CG_OK) { h->bslots = reinterpret_cast<double*>(h->bslots_base); h->sync_place = 0; return rc == CG_ETIMEOUT ? CG_OK : rc; }
+        if (k == 0 || c < best_c) { best = k; best_c = c; }
+    }
+    h->sync_place = best;
+    h->bslots = reinterpret_cast<double*>(h->bslots_base + (size_t)best * kBslotStep);
+    h->launches = 0;
+    return CG_OK;
+}
+
 extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
                          const int32_t* d_colind, const double* d_vals, void* d_workspace,
                          size_t workspace_bytes) {
@@ -723,7 +749,7 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
     h->rp_pad = (int*)w; w += rp_pad_bytes(n);
     h->part0 = (double*)w; w += kPartBytes; h->part1 = (double*)w; w += kPartBytes;
     h->part2 = (double*)w; w += kPartBytes; h->part3 = (double*)w; w += kPartBytes;
-    h->bslots = (double*)w; w += kBslotBytes;
+    h->bslots_base = w; h->bslots = (double*)w; w += kBslotReserve;
     h->scal = (Scal*)w; w += kScalBytes; h->dparams = (Params*)w; w += kParamBytes;
     static_assert(sizeof(Scal) <= kScalBytes && sizeof(Params) <= kParamBytes, "workspace slots");
     h->sms = prop.multiProcessorCount;
@@ -786,6 +812,8 @@ extern "C" int cg_create(cg_handle** out, int64_t n, int64_t nnz, const int32_t*
         for (const void* fn : shorts)
             if (fn) CKH(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin));
     }
+    rc = tune_sync_place(h);
+    if (rc != CG_OK) { cg_destroy(h); return rc; }
     *out = h;
     return CG_OK;
 }
@@ -1028,6 +1056,11 @@ static int set_option_one(cg_handle* h, const char* name, int64_t value) {
     if (!strcmp(name, "compress")) { if (value < 0 || value > 1) return CG_EINVAL; h->compress_opt = (int)value; drop_graph(); return CG_OK; }
     if (!strcmp(name, "fold")) { if (value < 0 || value > 2) return CG_EINVAL; h->fold_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "trace_clock")) { if (value < 0 || value > 1) return CG_EINVAL; h->trace_clock = (int)value; return CG_OK; }
+    if (!strcmp(name, "sync_place")) {
+        if (value < 0 || value > kBslotPlaces) return CG_EINVAL;
+        h->sync_place = (int)value; h->bslots = reinterpret_cast<double*>(h->bslots_base + (size_t)value * kBslotStep);
+        return CG_OK;
+    }
     if (!strcmp(name, "short_rows")) { if (value < 0 || value > 1) return CG_EINVAL; h->short_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "resident")) { if (value < 0 || value > 1) return CG_EINVAL; h->resident_opt = (int)value; return CG_OK; }
     if (!strcmp(name, "spin_budget_ms")) { if (value < 1 || value > 600000) return CG_EINVAL; h->spin_budget_ms = (int)value; return CG_OK; }
@@ -1071,6 +1104,8 @@ extern "C" int cg_get_info(cg_handle* h, const char* name, int64_t* value) {
     else if (!strcmp(name, "resident_rows")) *value = resident_rows(h, v);
     else if (!strcmp(name, "fold")) *value = fold_effective(h, v, 0, g) ? 1 : 0;
     else if (!strcmp(name, "algo")) *value = algo_effective(h, v, 0);
+    else if (!strcmp(name, "sync_place")) *value = h->sync_place;
+    else if (!strcmp(name, "sync_places")) *value = kBslotPlaces;
     else if (!strcmp(name, "short_rows")) *value = (short_rows_possible(h, v, g) && !(fold_effective(h, v, 0, g) && algo_effective(h, v, 0) == 0)) ? 1 : 0;
     else if (!strcmp(name, "compressed")) *value = (v >= 2 && g.cmp) ? 1 : 0;
     else if (!strcmp(name, "index_codes")) *value = h->idx_ready ? h->idx_codes : 0;
