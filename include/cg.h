@@ -29,7 +29,8 @@
  *    cg_strerror), -3 device not supported (needs compute capability 10.x),
  *    -4 device watchdog (a spin wait inside a solve ran out of its budget: a
  *    protocol error or a lost copy; the results of that call are void, the device
- *    is left usable), -5 out of host memory.
+ *    is left usable), -5 out of host memory, -6 size beyond what cg_dot_static's fixed
+ *    scratch can serve.
  *    Nothing is printed, thrown or aborted across this boundary.
  *  - The sparsity structure (rowptr, colind) is fixed for the life of the handle;
  *    vals may be rewritten between calls (then cg_set_option(h, "values_changed", 1)
@@ -58,6 +59,7 @@ typedef struct cg_handle cg_handle;
 #define CG_EUNSUPPORTED  -3
 #define CG_ETIMEOUT      -4
 #define CG_ENOMEM        -5
+#define CG_ETOOBIG       -6
 
 /* Bytes of device workspace cg_create needs for an n-row system: the vectors
  * r, p, q, one spare and D^-1 (each n doubles, 256-byte aligned), a padded copy of rowptr
@@ -133,6 +135,23 @@ int cg_spmv(cg_handle* h, const double* d_x, double* d_y, void* cuda_stream);
  * Synchronises the stream once. */
 int cg_dot(cg_handle* h, const double* d_a, const double* d_b,
            double* h_result, void* cuda_stream);
+
+/* The same scalar product for callers that may not allocate (code under CUDA
+ * graph capture, serving loops, harnesses that forbid cudaMalloc): no handle, no workspace, and
+ * no cudaMalloc / cudaFree / cudaHostAlloc / malloc on its path.  The per-block partial sums
+ * live in a fixed 32 KB __device__ array inside the library (held by every GPU that loads the
+ * library until the process exits), which bounds the size: n <= cg_dot_static_max_n() =
+ * 33 554 432; beyond that CG_ETOOBIG ("cg_dot_static: n exceeds ...").
+ * d_a, d_b: device double[n]; d_result: DEVICE double[1], written on the stream.  Asynchronous:
+ * nothing synchronises.  Blocks of 8192 elements, fixed-order sums: bitwise reproducible; the
+ * grouping differs from cg_dot's, so the two agree to rounding (1e-15 sum|a_i b_i| log2 n).
+ * Every call on a device shares the one scratch array: calls that may overlap on the GPU
+ * (different streams) race; calls on one stream are ordered.  A call reads only the partials
+ * it wrote itself, so nothing has to be cleared between calls.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress; make that
+ * call outside stream capture).  Errors: CG_EINVAL (n < 0, NULL), CG_ETOOBIG, CG_ECUDA. */
+int cg_dot_static(int64_t n, const double* d_a, const double* d_b, double* d_result, void* cuda_stream);
+int64_t cg_dot_static_max_n(void);
 
 /* Solve A x = b by unpreconditioned CG (readings in DESIGN.md):
  *   r = b - A x0; p = r; loop { q = A p; alpha = r.r / p.q; x += alpha p;

@@ -10,10 +10,10 @@ from .binding import (CG, CGError, CGResult, lib, cg_create, cg_destroy, cg_spmv
                       cg_solve_jacobi, cg_solve_host, cg_check_csr, cg_workspace_bytes,
                       cg_host_scratch_bytes, cg_set_option, cg_get_info, cg_strerror, cg_set_trace,
                       cg_probe_read_bandwidth, cg_index_bytes, cg_compress_index, cg_probe_grid_sync,
-                      cg_reorder_bytes, cg_reorder, cg_rcm_host)
+                      cg_reorder_bytes, cg_reorder, cg_rcm_host, cg_dot_static, cg_dot_static_max_n)
 
 __all__ = ["CG", "CGError", "CGResult", "lib", "cg_create", "cg_destroy", "cg_spmv", "cg_dot",
            "cg_solve", "cg_solve_jacobi", "cg_solve_host", "cg_check_csr", "cg_workspace_bytes",
            "cg_host_scratch_bytes", "cg_set_option", "cg_get_info", "cg_strerror", "cg_set_trace",
            "cg_probe_read_bandwidth", "cg_index_bytes", "cg_compress_index", "cg_probe_grid_sync",
-           "cg_reorder_bytes", "cg_reorder", "cg_rcm_host"]
+           "cg_reorder_bytes", "cg_reorder", "cg_rcm_host", "cg_dot_static", "cg_dot_static_max_n"]

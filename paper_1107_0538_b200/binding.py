@@ -32,6 +32,8 @@ SIGNATURES = {
     "cg_check_csr": (ctypes.c_int, [_vp, _vp]),
     "cg_spmv": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "cg_dot": (ctypes.c_int, [_vp, _vp, _vp, ctypes.POINTER(_f64), _vp]),
+    "cg_dot_static": (ctypes.c_int, [_i64, _vp, _vp, _vp, _vp]),
+    "cg_dot_static_max_n": (_i64, []),
     "cg_solve": (ctypes.c_int, [_vp, _vp, _vp, _f64, _i64, _vp, ctypes.POINTER(_i64),
                                 ctypes.POINTER(_f64), _vp]),
     "cg_solve_jacobi": (ctypes.c_int, [_vp, _vp, _vp, _f64, _i64, _vp, ctypes.POINTER(_i64),
@@ -148,6 +150,17 @@ def cg_dot(h: int, d_a: int, d_b: int, stream: int = 0) -> float:
     if rc != 0:
         raise CGError(rc, "cg_dot")
     return out.value
+
+
+def cg_dot_static(n: int, d_a: int, d_b: int, d_result: int, stream: int = 0) -> None:
+    """Handle-free, allocation-free dot product into DEVICE memory d_result; asynchronous on the stream."""
+    rc = lib().cg_dot_static(n, d_a, d_b, d_result, stream)
+    if rc != 0:
+        raise CGError(rc, "cg_dot_static")
+
+
+def cg_dot_static_max_n() -> int:
+    return int(lib().cg_dot_static_max_n())
 
 
 def _solve(fn_name, h, d_b, d_x, rtol, maxit, d_hist, stream):

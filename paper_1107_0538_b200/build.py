@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "cg_api.cu"), os.path.join(CSRC, "cg_variant.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("cg_kernels.cuh", "cg_stream.cuh", "cg_stream_kernels.cuh", "cg_variants.h", "cg_rcm.cpp")] \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("cg_kernels.cuh", "cg_stream.cuh", "cg_stream_kernels.cuh", "cg_variants.h", "cg_rcm.cpp", "cg_noalloc.cu")] \
     + [os.path.join(ROOT, "include", "cg.h")]
 LIB = os.path.join(HERE, "libcg_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
@@ -43,6 +43,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         units += [(f"shape{s}_cmp{c}", SOURCES[1], [f"-DCG_SHAPE={s}", f"-DCG_CMP={c}"]) for s in range(3) for c in range(2)]
         units += [("short", SOURCES[1], ["-DCG_SHORT"])]
         units += [("rcm", os.path.join(CSRC, "cg_rcm.cpp"), [])]
+        units += [("noalloc", os.path.join(CSRC, "cg_noalloc.cu"), [])]
         procs = []
         for name, src, defs in units:
             obj = os.path.join(tmp, name + ".o")

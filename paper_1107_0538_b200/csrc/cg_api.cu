@@ -841,6 +841,7 @@ extern "C" const char* cg_strerror(int code) {
         case CG_EUNSUPPORTED: return "device not supported (needs compute capability 10.x with cooperative launch)";
         case CG_ETIMEOUT: return "device watchdog: a spin wait inside the solve exceeded its budget; results are void";
         case CG_ENOMEM: return "out of host memory";
+        case CG_ETOOBIG: return "cg_dot_static: n exceeds the 33 554 432 elements its fixed scratch array can serve";
         default: return "unknown code";
     }
 }
