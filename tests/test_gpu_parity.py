@@ -340,6 +340,41 @@ def test_phase_trace_and_bandwidth_probe(bound, cgmod):
         cgmod.cg_probe_read_bandwidth(B.cg.h, 0, 1 << 20, 1, 0)
 
 
+def test_sync_place_and_global_clock_trace(bound, cgmod):
+    """Where the all-reduce inboxes sit ("sync_place", chosen by measurement at cg_create) cannot change a
+    bit of the result: the sums have one fixed order.  "trace_clock" = 1 stamps the nanosecond clock all SMs
+    share, so stamps of different CTAs are comparable: every CTA leaves a grid synchronisation after the last
+    one has reached it."""
+    B = bound(2)
+    p = B.p
+    for name, v in (("loop", 0), ("spmv", 0), ("algo", 0)):
+        B.cg.set_option(name, v)
+    places = B.cg.info("sync_places")
+    chosen = B.cg.info("sync_place")
+    assert places >= 200 and 0 <= chosen < 40
+    x0, r0 = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+    for place in (0, 7, places):
+        B.cg.set_option("sync_place", place)
+        assert B.cg.info("sync_place") == place
+        x, r = B.cg.solve(B.b, rtol=p.rtol, maxit=p.maxit)
+        assert r.iters == r0.iters and torch.equal(x, x0) and torch.equal(r.hist, r0.hist), place
+    with pytest.raises(cgmod.CGError):
+        B.cg.set_option("sync_place", places + 1)
+    B.cg.set_option("sync_place", chosen)
+    n_it = 12
+    B.cg.set_option("trace_clock", 1)
+    tr = B.cg.trace(n_it)
+    x, r = B.cg.solve(B.b, rtol=0.0, maxit=n_it)
+    t = tr.cpu().numpy().astype(np.int64)[:, 1:n_it - 1, :8]      # the last iteration leaves at the stop test
+    B.cg.trace(0)
+    B.cg.set_option("trace_clock", 0)
+    assert (np.diff(t, axis=2) >= 0).all()                                   # monotone inside an iteration
+    for arrive, leave in ((1, 2), (3, 4), (6, 7)):                             # the three synchronisations of the textbook loop
+        assert (t[:, :, leave].min(axis=0) >= t[:, :, arrive].max(axis=0)).all()
+    it_ns = float((t[:, -1, 7] - t[:, 0, 0]).mean()) / t.shape[1]
+    assert 3000.0 < it_ns < 100000.0                                           # ~10 us per iteration, in nanoseconds
+
+
 def test_graph_chunk_sizes_and_launch_count(bound):
     B = bound(0)
     p = B.p
