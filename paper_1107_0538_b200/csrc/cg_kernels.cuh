@@ -190,7 +190,8 @@ __device__ __forceinline__ bool grid_barrier(unsigned long long* bar, unsigned i
                 break;
             }
         }
-        __threadfence();                   // also invalidates this SM's L1 (CCTL.IVALL)
+        // no fence after the poll: the acquire loads pair with the other CTAs' release adds and invalidate
+        // this SM's L1 (CCTL.IVALL) themselves
     }
     return __syncthreads_or(dead) != 0;
 }

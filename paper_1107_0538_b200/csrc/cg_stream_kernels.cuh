@@ -631,8 +631,7 @@ __device__ __forceinline__ bool grid_barrier_partials(const Params& P, const Rin
             asm volatile("fence.acq_rel.gpu;" ::: "memory");
             asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(1ULL) : "memory");
             const unsigned long long target = (++nbar) * (unsigned long long)G;
-            bounded_spin(rg, [&] { return ld_relaxed_u64(ctr) >= target; });
-            asm volatile("fence.acq_rel.gpu;" ::: "memory");
+            bounded_spin(rg, [&] { return ld_acquire_u64(ctr) >= target; });      // acquire poll, as in grid_barrier_counter
             rg.red[kRedTot + kBarVals] = rg.ctl[4] != 0 ? 1.0 : 0.0;
         }
     }
