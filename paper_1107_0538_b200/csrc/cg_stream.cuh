@@ -133,12 +133,21 @@ template <int W> __device__ __forceinline__ void consumer_sync() {
     asm volatile("bar.sync 1, %0;" :: "n"(32 * W) : "memory");
 }
 
-// The CTA's contiguous tile range.
+// The CTA's contiguous tile range: floor(T / G) tiles each, and the T mod G tiles that are left over go to the
+// CTAs at the two ENDS of the matrix (half to the first ones, half to the last ones).  On a grid in natural ordering
+// those own the boundary planes, whose rows are shorter: at config 2 (4146 tiles = 148 x 28 + 2) the two 29-tile CTAs
+// used to sit mid-matrix, where every row is full, and the grid waited for them at every all-reduce (K1 7.5 k
+// against 7.0 k cycles).  For any other matrix the choice is as good as any.
+__device__ __forceinline__ long long cta_tile_begin(long long ntiles, int cta, int G) {
+    const long long q = ntiles / G, r = ntiles % G;
+    const long long head = (r + 1) / 2, tail = r / 2;         // CTAs [0, head) and [G - tail, G) own q + 1 tiles
+    const long long c = cta;
+    return c * q + (c < head ? c : head) + (c > G - tail ? c - (G - tail) : 0);
+}
 __device__ __forceinline__ void cta_tiles(const Params& P, int cta, int G, long long& tb, int& Tc) {
     const long long ntiles = (P.n + kTileRows - 1) / kTileRows;
-    tb = (long long)cta * ntiles / G;
-    const long long te = (long long)(cta + 1) * ntiles / G;
-    Tc = (int)(te - tb);
+    tb = cta_tile_begin(ntiles, cta, G);
+    Tc = (int)(cta_tile_begin(ntiles, cta + 1, G) - tb);
 }
 
 // ---------------------------------------------------------------- watchdog
