@@ -206,3 +206,42 @@ def test_reorder_declined_on_a_well_numbered_matrix(problems):
     x, res = A.solve(_dev(p.b), rtol=p.rtol, maxit=p.maxit)
     assert res.status == 0 and A.info("launches") == 1
     A.close()
+
+
+@pytest.mark.gpu
+def test_reorder_with_rows_longer_than_the_sorting_limit(problems):
+    """A 14^3 stencil plus one node coupled to the 400 nodes around it (a local 'arrow'), then randomly
+    permuted: that row (and no other) is longer than the 256 entries cg_reorder sorts in registers, so it
+    keeps its stored order; the renumbering is still taken, and the solve must match the oracle within the
+    bands in both numberings."""
+    import scipy.sparse as sp
+    import paper_1107_0538_b200 as cg
+    from oracle import cg_oracle as orc
+    p = problems(2, 14)
+    n = p.n
+    A0 = sp.csr_matrix((p.vals, p.colind, p.rowptr), shape=(n, n))
+    rng = np.random.default_rng(7)
+    hub = n // 2
+    others = np.setdiff1d(np.arange(hub - 200, hub + 201), [hub])
+    w = 1e-3 * (1.0 + rng.random(len(others)))
+    arrow = sp.coo_matrix((np.concatenate([-w, -w]), (np.concatenate([np.full(len(others), hub), others]),
+                                                       np.concatenate([others, np.full(len(others), hub)]))), shape=(n, n))
+    diag = np.zeros(n)
+    diag[hub] = w.sum()
+    diag[others] = w
+    A = (A0 + arrow + sp.diags(diag)).tocsr()                 # still symmetric and strictly diagonally dominant
+    perm = rng.permutation(n)
+    A = A[perm][:, perm].tocsr()
+    A.sort_indices()
+    rp, ci, va = A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(np.float64)
+    assert np.diff(rp).max() > 256
+    b = cg_inputs.seeded_vector(21, n)
+    ref = orc.cg(rp, ci, va, b, rtol=1e-10, maxit=n)
+    H = cg.CG(_dev(rp), _dev(ci), _dev(va), reorder=False)
+    x0, r0 = H.solve(_dev(b), rtol=1e-10, maxit=n)
+    _parity(r0, x0, ref)
+    assert H.reorder() and H.info("reordered") == 1           # kept: the gathers become more local
+    x1, r1 = H.solve(_dev(b), rtol=1e-10, maxit=n)
+    _parity(r1, x1, ref)
+    assert H.info("launches") == 3
+    H.close()
