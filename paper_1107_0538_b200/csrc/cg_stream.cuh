@@ -7,7 +7,7 @@
 // partials, K3 p = r + beta p, scalars on the device.
 //
 // Work split.  The matrix is cut into tiles of 32 consecutive rows.  CTA c owns the
-// contiguous tiles [c*T/G, (c+1)*T/G); inside a CTA tile j (0-based) belongs to consumer warp
+// contiguous tiles (cta_tiles below: T/G each, the left-over tiles at the two ends); inside a CTA tile j (0-based) belongs to consumer warp
 // j mod W, lane l of that warp owns row 32*tile + l in EVERY phase.  The thread that
 // computes q_i is therefore the thread that updates x_i, r_i, p_i, and all per-thread
 // partial sums are accumulated in tile order: every loop mode (persistent with vectors in

@@ -604,7 +604,7 @@ __global__ void __launch_bounds__(Shape<W, NP>::kThreads, 1) ks_persistent_cg1(P
 //     beta = gamma / gamma_old ; alpha = gamma / (delta - beta gamma / alpha_old)
 //     z = q + beta z ; s = w + beta s ; p = r + beta p ; x += alpha p ; r -= alpha s ; w -= alpha z
 //     -- counter barrier: w and the partials are published --
-// One grid synchronisation per iteration: the counter barrier's release / acquire fences make
+// One grid synchronisation per iteration: the counter barrier's release fence and acquire polls make
 // every CTA's partials (one plain store per CTA and value, double-buffered by iteration parity)
 // visible to everyone who leaves the barrier, so the "all-reduce" is 148 L2 reads per value that
 // every warp issues after its K1 tiles and sums in one fixed order: nobody polls, and the
