@@ -705,7 +705,9 @@ static int tune_sync_place(cg_handle* h) {
         h->bslots = reinterpret_cast<double*>(h->bslots_base + (size_t)k * kBslotStep);
         double c = 0.0;
         const int rc = cg_probe_grid_sync(h, 1, kTuneReps, &c, nullptr);
-        if (rc != CG_OK) { h->bslots = reinterpret_cast<double*>(h->bslots_base); h->sync_place = 0; return rc == CG_ETIMEOUT ? CG_OK : rc; }
+        // the placement is an optimisation: if the probe cannot run (no room for a cooperative launch right now, a
+        // watchdog trip, ...) the inboxes stay at the start of the reserve and cg_create goes on
+        if (rc != CG_OK) { cudaGetLastError(); h->bslots = reinterpret_cast<double*>(h->bslots_base); h->sync_place = 0; h->launches = 0; return CG_OK; }
         if (k == 0 || c < best_c) { best = k; best_c = c; }
     }
     h->sync_place = best;
