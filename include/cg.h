@@ -212,9 +212,9 @@ int cg_solve_host(cg_handle* h, const double* h_b, double* h_x,
  *               1 = fold K3 into the next K1 (every gathered p_j is recomputed on the fly as
  *               fma(beta, p_old_j, r_j) from one 16-byte {p_old, r} pair, the owner's own
  *               expression, so results keep their bits) and synchronise the grid twice
- *               instead of three times per iteration; 0 = off; 2 (default) = on when a CTA
- *               gathers <= 500 entries per lane-row set (tiles x mean row length) and the
- *               short-row kernels do not apply
+ *               instead of three times per iteration; 0 = off; 2 (default) = on when no row has
+ *               more than 9 entries, a CTA gathers <= 500 entries per lane (tiles x mean row
+ *               length) and the short-row kernels do not apply
  *   "sync_place" where the all-reduce inboxes sit in their reserve, in steps of 64 KB
  *               (0 .. cg_get_info "sync_places"); cg_create picks it by measurement
  *   "short_rows" 1 (default) = when no row has more than 9 entries (the 7-point Laplacian), every

@@ -652,11 +652,12 @@ static bool fold_effective(const cg_handle* h, int v, int precond, const Geo& g)
     if (h->fold_opt != 2) return h->fold_opt == 1;
     // auto: where the short-row kernels apply they win (config 1: 8.9 against 10.6 us per iteration folded)
     if (short_rows_possible(h, v, g)) return false;
-    // auto: the 16-byte gathers must cost less than the synchronisation they save.  Measured
-    // (us per iteration, folded / not): config 0 (1 tile of 24 entries per row per CTA) 7.4 / 7.8,
-    // config 1 (56 pinned tiles x 7) 10.6 / 13.4, config 2 (29 pinned tiles x 26) 10.8 / 10.4.
+    // auto: the 16-byte gathers must cost less than the synchronisation they save.  Since the counter
+    // barrier polls with acquire loads that is only so for short rows on small systems.  Measured (us per
+    // iteration, folded / not): 27-point 16^3 7.27 / 6.92, 24^3 7.32 / 6.90, 32^3 7.48 / 7.16, 40^3 8.26 / 7.72,
+    // 51^3 (config 2) 11.0 / 9.5; 7-point 32^3 6.68 / 6.88, 48^3 7.88 / 7.66 (short-row kernel), 64^3 10.6 / 8.7.
     const double gathers = (double)tiles_per_cta_max(h) * (double)h->nnz / (double)h->n;
-    return gathers <= 500.0;
+    return h->max_row_len <= 9 && gathers <= 500.0;
 }
 
 // Options "algo" = 1 (Chronopoulos-Gear) and 2 (pipelined CG) apply to the persistent streamed
